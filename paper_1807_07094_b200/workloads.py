@@ -117,7 +117,7 @@ def gaussian_field(N, rng, kmax=None):
     amp[m] = 1.0 / k[m]
     if kmax is not None:
         amp[k > kmax] = 0.0
-    g = np.fft.irfftn(fk * amp, s=(N, N, N))
+    g = np.fft.irfftn(fk * amp, s=(N, N, N), axes=(0, 1, 2))
     g -= g.mean()
     g /= g.std()
     return g

@@ -1,0 +1,160 @@
+"""Pins for the oracle's chemistry/thermal update (O6) and for trace+chemistry together
+(the analytic Stromgren sphere)."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_1807_07094_b200 import workloads as wl
+
+GOLD = dict(l.split()[:2] for l in open(__file__.rsplit("/", 1)[0] + "/golden/paper_values.txt")
+            if l.strip() and not l.startswith("#"))
+
+
+def _params(w, **kw):
+    return orc.make_params(w, **kw)
+
+
+def test_alpha_B_reproduces_the_papers_trec_and_stromgren_radius():
+    # n_H = 1e-3, T = 1e4 K, Ndot = 5e48  ->  t_rec = 122.4 Myr, R_S = 5.4 kpc
+    aB = orc.rate_coeffs(1e4, caseB=1)[0]
+    nH, Nd = float(GOLD["test1_nH"]), float(GOLD["test1_Ndot"])
+    t_rec = 1.0 / (aB * nH) / wl.MYR_S
+    R_S = (3 * Nd / (4 * math.pi * aB * nH ** 2)) ** (1 / 3) / wl.KPC_CM
+    assert abs(t_rec / float(GOLD["recombination_time_myr"]) - 1) < 2e-3
+    assert abs(R_S - float(GOLD["stromgren_radius_kpc"])) < 0.05
+    assert abs(aB / wl.ALPHA_B_1E4 - 1) < 2e-3
+
+
+def test_rate_coefficients_sanity():
+    # not pinned by the paper ("parity unpinned"); physical sanity only
+    for T in (1e2, 1e3, 1e4, 1e5, 1e6):
+        a = orc.rate_coeffs(T, caseB=0)
+        b = orc.rate_coeffs(T, caseB=1)
+        assert np.all(a >= 0) and np.all(b >= 0) and np.all(np.isfinite(a))
+        assert b[0] < a[0] and b[2] < a[2]                       # case B < case A
+    assert orc.rate_coeffs(2e4)[0] < orc.rate_coeffs(1e4)[0]     # recombination falls with T
+    assert orc.rate_coeffs(2e4)[3] > orc.rate_coeffs(1e4)[3]     # collisional ionisation rises with T
+    assert np.all(orc.rate_coeffs(1e4, coll_ion=0)[3:6] == 0)
+    # collisional-ionisation equilibrium of H at 1e4 K is a small ionised fraction (PAPER.md:268 quotes 1.2e-3)
+    c = orc.rate_coeffs(1e4, caseB=0)
+    assert 1e-4 < c[3] / c[0] < 1e-2
+
+
+def test_one_bdf_step_is_the_backward_difference_formula():
+    w = wl.config2(4)
+    p = _params(w, max_subcycles=1)
+    aB = orc.rate_coeffs(1e4)[0]
+    nH, x0, G, dt = 1e-3, 0.7, 3e-13, 4e13
+    x, T, k = orc.chem_cell(p, nH, [x0, 1.0, 0.0], 1e4, [G, 0, 0], [0, 0, 0], dt)
+    ne = nH * (1 - x0)
+    D, Cc = aB * ne * (1 - x0), G
+    assert k == 1 and T == 1e4
+    assert abs(x[0] - (x0 + D * dt) / (1 + Cc * dt)) < 1e-15
+    # dt -> infinity: n -> D/C
+    x, _, _ = orc.chem_cell(p, nH, [x0, 1.0, 0.0], 1e4, [G, 0, 0], [0, 0, 0], 1e30)
+    assert abs(x[0] - D / Cc) < 1e-12
+
+
+def test_recombination_only_closed_form():
+    # Gamma = 0, C = 0, fixed T, pure H: dx/dt = -alpha n_H x^2  ->  x(t) = x0/(1 + x0 alpha n_H t)
+    w = wl.config2(4)
+    aB = orc.rate_coeffs(1e4)[0]
+    nH, xi0 = 1e-3, 0.9
+    t = 2.0 / (aB * nH)
+    exact = xi0 / (1 + xi0 * aB * nH * t)
+    errs = []
+    for eps in (0.1, 0.01, 0.001):
+        p = _params(w, eps_sub=eps, max_subcycles=1000000)
+        x, _, k = orc.chem_cell(p, nH, [1 - xi0, 1.0, 0.0], 1e4, [0, 0, 0], [0, 0, 0], t)
+        errs.append(abs((1 - x[0]) - exact) / exact)
+    assert errs[2] < 2e-3 and errs[2] < errs[1] < errs[0]        # first-order convergence to the closed form
+
+
+def test_photoionisation_equilibrium_root():
+    # constant Gamma: Gamma x_HI = alpha n_H (1 - x_HI)^2
+    w = wl.config2(4)
+    aB = orc.rate_coeffs(1e4)[0]
+    nH, G = 1e-3, 1e-13
+    a = aB * nH
+    # a(1-x)^2 - G x = 0
+    xr = ((2 * a + G) - math.sqrt((2 * a + G) ** 2 - 4 * a * a)) / (2 * a)
+    p = _params(w)
+    x = [1.0 - 1.2e-3, 1.0, 0.0]
+    for _ in range(40):
+        x, _, _ = orc.chem_cell(p, nH, list(x), 1e4, [G, 0, 0], [0, 0, 0], 5.0 / a)
+    assert abs(x[0] / xr - 1) < 1e-6
+
+
+def test_fractions_stay_physical_and_helium_closes():
+    rng = np.random.default_rng(0)
+    w = wl.tiny(N=4, nb=3)
+    p = _params(w)
+    for _ in range(300):
+        nH = 10 ** rng.uniform(-4, 0)
+        xHeI = rng.uniform(0, 1)
+        x0 = [rng.uniform(0, 1), xHeI, (1 - xHeI) * rng.uniform(0, 1)]
+        G = 10 ** rng.uniform(-16, -9, 3)
+        H = G * rng.uniform(1, 30) * 1.6e-12
+        T0 = 10 ** rng.uniform(1, 5)
+        x, T, k = orc.chem_cell(p, nH, x0, T0, G, H, 10 ** rng.uniform(10, 15))
+        assert np.all(x >= 0) and np.all(x <= 1) and x[1] + x[2] <= 1 + 1e-15
+        assert 1.0 <= T < 1e6 and 1 <= k <= p.max_subcycles
+
+
+def test_thermal_equilibrium_is_around_1e4_K():
+    # photo-heated pure-H gas settles near 1-2e4 K ("temperatures above 2e4 K is rare")
+    w = wl.config2(4)
+    p = _params(w, isothermal=0, coll_ion=1, caseB=1)
+    x, T = [1.0 - 1.2e-3, 1.0, 0.0], 100.0
+    G = 1e-12
+    for _ in range(50):
+        x, T, _ = orc.chem_cell(p, 1e-3, list(x), T, [G, 0, 0], [G * 3.4 * 1.602e-12 * 0 + G * 5.0e-12, 0, 0], 3e14)
+    assert 5e3 < T < 4e4 and x[0] < 0.05
+
+
+def _stromgren_run(N, nsteps, dtfrac):
+    w = wl.config2(N)
+    aB = orc.rate_coeffs(1e4)[0]
+    t_rec = 1.0 / (aB * 1e-3)
+    R_S = (3 * 5e48 / (4 * math.pi * aB * 1e-6)) ** (1 / 3)
+    dx = w.box_cm / N
+    f = tuple(np.asarray(a, dtype=np.float64) for a in w.fields())
+    ratios, radii = [], []
+    for s in range(nsteps):
+        out = orc.step(w, f, dt=dtfrac * t_rec)
+        f = out["fields"]
+        t = (s + 1) * dtfrac * t_rec
+        xe = (1.0 - f[1] - 1.2e-3).clip(0)                     # above the initial ionised background
+        rV = (3 * xe.sum() * dx ** 3 / (4 * math.pi)) ** (1 / 3)
+        ra = R_S * (1 - math.exp(-t / t_rec)) ** (1 / 3)       # Eq. 9 (reading G1)
+        ratios.append(rV / ra); radii.append(rV)
+        em, ab, es = out["stats"]["emitted"], out["stats"]["absorbed"], out["stats"]["escaped"]
+        assert abs((ab[0] + es[0]) / em[0] - 1) < 1e-10
+    return np.array(ratios), np.array(radii), R_S, f, w
+
+
+def test_stromgren_small_steps_follows_eq9():
+    ratios, radii, R_S, f, w = _stromgren_run(32, 300, 0.01)
+    t = (np.arange(300) + 1) * 0.01
+    assert np.all(np.diff(radii) > 0)                           # monotone growth
+    late = ratios[t >= 0.8]
+    assert np.all(np.abs(late - 1) < 0.05), (late.min(), late.max())
+    assert abs(ratios[-1] - 1) < 0.03
+    # sharp front: x_HI goes from < 0.1 to > 0.9 within a few cells along +x from the source
+    N = 32
+    x3 = f[1].reshape(N, N, N)
+    line = x3[N // 2, N // 2, N // 2:]
+    i_in = np.max(np.flatnonzero(line < 0.1)); i_out = np.min(np.flatnonzero(line > 0.9))
+    assert 0 < i_out - i_in <= 4
+
+
+def test_stromgren_coarse_steps_reaches_the_papers_accuracy():
+    # config 2's stepping (100 steps of 0.05 t_rec) at 32^3: lags early, final radius within
+    # the 5 % the paper reports
+    ratios, radii, R_S, f, w = _stromgren_run(32, 100, 0.05)
+    assert np.all(np.diff(radii) > 0)
+    assert ratios[0] < 0.5                                       # the fixed-step lag the paper describes
+    assert abs(ratios[-1] - 1) < float(GOLD["stromgren_accuracy"])
+    assert abs(radii[-1] / R_S / (1 - math.exp(-5)) ** (1 / 3) - 1) < 0.05
