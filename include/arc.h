@@ -1,0 +1,165 @@
+/* arc.h -- C ABI of the B200-native ARC hot path (libarc_b200.so).
+ *
+ * ARC = photon-conserving, spatially adaptive HEALPix ray tracing from point sources through a
+ * uniform N^3 grid, followed by the per-cell ionisation/heating update (Hartley & Ricotti 2018,
+ * arXiv:1807.07094; citations below are PAPER.md line numbers, and DESIGN.md for the readings
+ * where the paper is silent).
+ *
+ * Conventions
+ *  - every call returns an int status (ARC_OK = 0, negative = error); nothing throws or aborts;
+ *    arc_last_error() gives the text of the last failure of that context.
+ *  - all grid arrays are C-contiguous, x fastest: index = (iz*N + iy)*N + ix.  Units are cgs;
+ *    photon energies in eV.
+ *  - `where` says where caller pointers live: ARC_HOST (pageable or pinned host memory) or
+ *    ARC_DEVICE (device memory of the current CUDA device).  Inputs are COPIED: the caller keeps
+ *    ownership of everything it passes in.  Device pointers handed OUT (arc_rates) are owned by the
+ *    library and stay valid until the next arc_trace() or arc_destroy() on that context.
+ *  - every step of the path runs in CUDA kernels for sm_100a; there is no CPU fallback.  Without a
+ *    CUDA device arc_create_grid() returns ARC_ECUDA.
+ *  - work is enqueued on the stream given to arc_set_stream() (default: the legacy default stream).
+ *    With arc_params.async == 0 (default) arc_trace()/arc_update_chemistry() synchronise that
+ *    stream before returning and report device-side errors (e.g. ARC_EOVERFLOW) themselves; with
+ *    async == 1 they only enqueue, and deferred errors surface from arc_synchronize()/arc_get_stats().
+ */
+#ifndef ARC_B200_H
+#define ARC_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ARC_MAX_BINS 8
+#define ARC_MAX_LEVEL 16
+
+typedef struct arc_ctx arc_ctx;                       /* opaque; owns all device memory */
+
+enum { ARC_F32 = 0, ARC_F64 = 1 };                    /* dtype of the five gas fields */
+enum { ARC_HOST = 0, ARC_DEVICE = 1 };
+enum { ARC_OK = 0, ARC_EINVAL = -1, ARC_ENOMEM = -2, ARC_ECUDA = -3, ARC_ESTATE = -4, ARC_EOVERFLOW = -5 };
+enum { ARC_END_SPLIT = 0, ARC_END_DEPLETED = 1, ARC_END_ESCAPED = 2 };
+
+/* Free parameters the paper names (PAPER.md:45 initial level, :96/:348 Phi, :154 eps; G7
+ * tau_term) plus run-time switches of this implementation. */
+typedef struct arc_params {
+    int32_t l0;             /* initial HEALPix level: 12*4^l0 root rays per source      */
+    int32_t Lmax;           /* rays at this level never split; <= 14 (pixel ids are 32 bit)          */
+    double  Phi;            /* rays per cell: split when Omega_l r^2 > dx^2/Phi   */
+    double  tau_term;       /* ray ends when min_nu tau_nu >= tau_term (+inf disables)               */
+    double  Yp;             /* helium mass fraction; 0 = pure hydrogen              */
+    int32_t isothermal;     /* 1: T fixed, energy equation skipped                                   */
+    int32_t caseB;          /* 1: case-B recombination coefficients                                  */
+    int32_t coll_ion;       /* 1: collisional ionisation terms C_S(T) of Eq. 4 on                    */
+    int32_t max_subcycles;  /* cap on chemistry sub-cycles per cell per call                         */
+    double  eps_sub;        /* sub-cycle fractional change, 0.1 in the paper          */
+    double  x_floor;        /* lower clamp of x_HI, x_HeI                                            */
+    int32_t digest;         /* 1: also accumulate the order-independent traversal digest (slower)    */
+    int32_t async;          /* 1: arc_trace/arc_update_chemistry do not synchronise (see top)        */
+    int32_t trace_blocks;   /* persistent-kernel grid size; 0 = SM count x resident blocks per SM    */
+    int32_t reserved;
+} arc_params;
+
+/* Per-cell outputs of arc_trace (PAPER.md:83 Eq. 1, :134-138, :170): DEVICE pointers, N^3 doubles each. */
+typedef struct arc_rates {
+    const double *Gamma_HI, *Gamma_HeI, *Gamma_HeII;   /* photo-ionisation rate per absorber [1/s]     */
+    const double *heat_HI, *heat_HeI, *heat_HeII;      /* photo-heating per absorber [erg/s]           */
+    const double *heat_total;                          /* sum_S heat_S n_S [erg/s/cm^3] */
+} arc_rates;
+
+typedef struct arc_stats {
+    uint64_t segments;                 /* (ray, cell) deposit events of the last arc_trace             */
+    uint64_t rays;                     /* ray records traced (all levels)                              */
+    uint64_t digest;                   /* sum mod 2^64 of per-ray hashes (only if params.digest)       */
+    uint64_t queue_high_water;         /* max entries seen in the global donation queue                */
+    uint64_t splits[ARC_MAX_LEVEL];    /* rays that split, per level                                   */
+    uint64_t rays_level[ARC_MAX_LEVEL];
+    uint64_t ends[3];                  /* rays ended by ARC_END_*                                      */
+    double   emitted[ARC_MAX_BINS];    /* photons/s per bin: sum over sources                          */
+    double   absorbed[ARC_MAX_BINS];   /* = sum over cells of the accumulators                         */
+    double   escaped[ARC_MAX_BINS];    /* left the box ("radiation leaving the box is lost") */
+    uint64_t subcycles;                /* total chemistry sub-cycles of the last arc_update_chemistry  */
+    uint32_t max_subcycles_cell;       /* largest per-cell sub-cycle count of that call                */
+    uint32_t pad;
+    float    trace_ms, chem_ms;        /* CUDA-event durations of the last calls (whole call, on-stream) */
+    float    trace_kernel_ms;          /* the persistent ray-tracing kernel alone (same events, same stream) */
+    float    opacity_ms, finalize_ms;  /* the two per-cell passes around it                               */
+    int32_t  trace_grid;               /* thread blocks of the persistent kernel                          */
+} arc_stats;
+
+/* Caller-provided HOST buffers for arc_trace_debug: one entry per segment (seq = 0,1,2,... within the
+ * ray, cell = linear cell index) and one closing entry per ray (seq = number of segments,
+ * cell = -1 - ARC_END_*).  key = (src << 40) | (level << 32) | pixel.  Entries arrive unordered. */
+typedef struct arc_raylog {
+    int64_t   cap;        /* capacity of the three arrays (entries)                                    */
+    int64_t   n;          /* out: entries written                                                      */
+    uint64_t *key;
+    uint32_t *seq;
+    int32_t  *cell;
+} arc_raylog;
+
+/* Grid of N^3 cells in a cube of side box_cm.  dtype = ARC_F32 | ARC_F64 is the storage
+ * type of the five gas fields and of the per-step opacity table; accumulators and rates are fp64.
+ * Errors: ARC_EINVAL (N < 1 or N > 1024, box <= 0, bad dtype), ARC_ECUDA (no device), ARC_ENOMEM. */
+int arc_create_grid(arc_ctx **out, int N, double box_cm, int dtype);
+int arc_destroy(arc_ctx *c);
+
+void arc_default_params(arc_params *p);                /* l0=1, Phi=3, Lmax=13, tau_term=30, eps=0.1 ... */
+int arc_set_params(arc_ctx *c, const arc_params *p);   /* ARC_EINVAL on out-of-range values             */
+int arc_set_stream(arc_ctx *c, void *cuda_stream);     /* cudaStream_t; NULL = default stream           */
+
+/* Gas fields: n_H [cm^-3], neutral/ionised fractions x_HI, x_HeI, x_HeII, T [K]; each
+ * N^3 values of the grid dtype.  x_HeII is this build's third absorber (G12). */
+int arc_set_fields(arc_ctx *c, const void *n_H, const void *x_HI, const void *x_HeI,
+                   const void *x_HeII, const void *T, int where);
+int arc_get_fields(arc_ctx *c, void *n_H, void *x_HI, void *x_HeI, void *x_HeII, void *T, int where);
+                                                       /* NULL pointers are skipped */
+
+/* Frequency bins: per bin one representative energy and one frequency-averaged
+ * cross-section per species [cm^2].  1 <= nbins <= ARC_MAX_BINS.  HOST pointers. */
+int arc_set_spectrum(arc_ctx *c, int nbins, const double *E_eV, const double *sig_HI,
+                     const double *sig_HeI, const double *sig_HeII);
+
+/* Point sources: position [cm] in [0, box) on every axis (else ARC_EINVAL), photon
+ * rate Ndot [1/s] and its split over the bins (rows of binfrac).  HOST pointers.  Call after
+ * arc_set_spectrum (ARC_ESTATE otherwise). */
+int arc_set_sources(arc_ctx *c, int nsrc, const double *pos_cm /*[nsrc][3]*/, const double *Ndot,
+                    const double *binfrac /*[nsrc][nbins]*/);
+
+/* One radiative-transfer pass (PAPER.md:47-56 steps i, iii; :79-98; Eq. 1): zero the accumulators,
+ * rebuild the opacity table from the current fields, trace every ray of every source (persistent
+ * kernel), finalise the per-cell rates.  `step` is a label only.  out may be NULL.
+ * Errors: ARC_ESTATE (fields / spectrum / sources missing), ARC_EOVERFLOW (work stack or queue
+ * exhausted: rates invalid), ARC_ECUDA. */
+int arc_trace(arc_ctx *c, int step, arc_rates *out);
+
+/* Copy the rates out: each non-NULL pointer receives N^3 doubles (host or device per `where`). */
+int arc_get_rates(arc_ctx *c, double *Gamma_HI, double *Gamma_HeI, double *Gamma_HeII,
+                  double *heat_HI, double *heat_HeI, double *heat_HeII, double *heat_total, int where);
+
+/* Raw accumulators of the last trace: absorbed photons/s, layout [cell][bin], N^3*nbins doubles. */
+int arc_get_accum(arc_ctx *c, double *A, int where);
+
+/* Sub-cycled backward-difference update of x_HI, x_HeI, x_HeII, T over dt_s with the rates of the
+ * last arc_trace held fixed (PAPER.md:57 step v; :136-154 Eq. 4-5; :166-172).  ARC_ESTATE if no
+ * trace has been done since the fields were last set. */
+int arc_update_chemistry(arc_ctx *c, double dt_s);
+
+int arc_synchronize(arc_ctx *c);                       /* wait for the stream; report deferred errors */
+int arc_get_stats(arc_ctx *c, arc_stats *s);           /* synchronises */
+
+/* Same as arc_trace but with per-ray logging into caller-provided host buffers (small configs only).
+ * ARC_EOVERFLOW if log->cap is too small (log->n then holds the number needed, if known). */
+int arc_trace_debug(arc_ctx *c, int step, arc_raylog *log);
+
+/* Device HEALPix generator, exposed for testing (O1): unit vectors of `n` (level, pixel) pairs.
+ * HOST pointers; out is [n][3]. */
+int arc_pix2vec(const int32_t *level, const uint32_t *pix, int n, double *out);
+
+const char *arc_last_error(const arc_ctx *c);          /* c may be NULL: last error of a failed create */
+const char *arc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,127 @@
+// arc_fields.cu -- per-cell streaming kernels around the tracer.
+//   a1+a2 fused: zero the accumulators and build the opacity table
+//           kappa_nu = (sigma_HI,nu n_HI + sigma_HeI,nu n_HeI) + sigma_HeII,nu n_HeII
+//         evaluated in fp64 left to right and rounded to the field dtype (O4).
+//   a10: finalise  Gamma_S = (1/V) sum_nu A_nu sigma_S,nu / kappa'_nu,  heat_S likewise with (E_nu - E_S)
+//         (Eq. 1 with n_abs = n_SI; species share = opacity share, reading G8).
+// SoA fields (5 arrays at the field dtype) are read fully coalesced, one cell per thread.
+#include "arc_internal.cuh"
+
+namespace {
+
+__device__ __forceinline__ double n_helium(double nH, double Yp) { return nH * Yp / (4.0 * (1.0 - Yp)); }
+
+template <typename FT>
+__global__ void __launch_bounds__(256) arc_opacity_kernel(long long ncell, int nb, double Yp, Spectrum sp,
+                                                         const FT *__restrict__ nH, const FT *__restrict__ xHI,
+                                                         const FT *__restrict__ xHeI, const FT *__restrict__ xHeII,
+                                                         FT *__restrict__ kappa, double *__restrict__ A)
+{
+    for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
+        const double n = (double)nH[c];
+        const double nHe = n_helium(n, Yp);
+        const double nHI = __dmul_rn(n, (double)xHI[c]);
+        const double nHeI = __dmul_rn(nHe, (double)xHeI[c]);
+        const double nHeII = __dmul_rn(nHe, (double)xHeII[c]);
+        for (int v = 0; v < nb; ++v) {
+            const double k = __dadd_rn(__dadd_rn(__dmul_rn(sp.sig[0][v], nHI), __dmul_rn(sp.sig[1][v], nHeI)),
+                                       __dmul_rn(sp.sig[2][v], nHeII));
+            kappa[c * nb + v] = (FT)k;
+            A[c * nb + v] = 0.0;
+        }
+    }
+}
+
+template <typename FT>
+__global__ void __launch_bounds__(256) arc_finalize_kernel(long long ncell, int nb, double Yp, double V, Spectrum sp,
+                                                          const FT *__restrict__ nH, const FT *__restrict__ xHI,
+                                                          const FT *__restrict__ xHeI, const FT *__restrict__ xHeII,
+                                                          const double *__restrict__ A, double *__restrict__ rates,
+                                                          double *__restrict__ absorbed)
+{
+    const double EV = 1.602176634e-12;
+    const double ETH[3] = {13.598, 24.587, 54.418};
+    double acc[ARC_MAX_BINS];
+#pragma unroll
+    for (int v = 0; v < ARC_MAX_BINS; ++v) acc[v] = 0.0;
+    for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
+        const double n = (double)nH[c];
+        const double nHe = n_helium(n, Yp);
+        const double ns[3] = {n * (double)xHI[c], nHe * (double)xHeI[c], nHe * (double)xHeII[c]};
+        double G[3] = {0.0, 0.0, 0.0}, H[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+        for (int v = 0; v < ARC_MAX_BINS; ++v) {
+            if (v >= nb) break;
+            const double Av = A[c * nb + v];
+            acc[v] += Av;
+            const double kp = (sp.sig[0][v] * ns[0] + sp.sig[1][v] * ns[1]) + sp.sig[2][v] * ns[2];
+            if (kp > 0.0) {
+                const double w = Av / (V * kp);
+#pragma unroll
+                for (int S = 0; S < 3; ++S) {
+                    const double ws = w * sp.sig[S][v];
+                    G[S] += ws;
+                    if (sp.E[v] > ETH[S]) H[S] += ws * ((sp.E[v] - ETH[S]) * EV);
+                }
+            }
+        }
+#pragma unroll
+        for (int S = 0; S < 3; ++S) { rates[S * ncell + c] = G[S]; rates[(3 + S) * ncell + c] = H[S]; }
+        rates[6 * ncell + c] = (H[0] * ns[0] + H[1] * ns[1]) + H[2] * ns[2];
+    }
+    // stats: absorbed_nu = sum over cells of A_nu (photon-conservation check)
+    __shared__ double sm[ARC_MAX_BINS][8];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int v = 0; v < ARC_MAX_BINS; ++v) {
+        double x = acc[v];
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+        if (lane == 0) sm[v][w] = x;
+    }
+    __syncthreads();
+    if (threadIdx.x < nb) {
+        double x = 0.0;
+        for (int i = 0; i < 8; ++i) x += sm[threadIdx.x][i];
+        atomicAdd(absorbed + threadIdx.x, x);
+    }
+}
+
+}  // namespace
+
+static int stream_grid(arc_ctx *c, long long n)
+{
+    long long b = (n + 255) / 256;
+    const long long cap = (long long)c->n_sm * 16;      // grid-stride: a multiple of the SM count
+    return (int)(b < cap ? b : cap);
+}
+
+cudaError_t arc_launch_opacity(arc_ctx *c)
+{
+    const int g = stream_grid(c, c->ncell);
+    if (c->dtype == ARC_F32)
+        arc_opacity_kernel<float><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, c->p.Yp, c->spec, (const float *)c->f[0],
+                                                          (const float *)c->f[1], (const float *)c->f[2], (const float *)c->f[3],
+                                                          (float *)c->d_kappa, c->d_A);
+    else
+        arc_opacity_kernel<double><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, c->p.Yp, c->spec, (const double *)c->f[0],
+                                                           (const double *)c->f[1], (const double *)c->f[2], (const double *)c->f[3],
+                                                           (double *)c->d_kappa, c->d_A);
+    return cudaGetLastError();
+}
+
+cudaError_t arc_launch_finalize(arc_ctx *c)
+{
+    cudaError_t e = cudaMemsetAsync(c->d_absorbed, 0, sizeof(double) * ARC_MAX_BINS, c->stream);
+    if (e != cudaSuccess) return e;
+    const int g = stream_grid(c, c->ncell);
+    const double V = c->dx * c->dx * c->dx;
+    if (c->dtype == ARC_F32)
+        arc_finalize_kernel<float><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, c->p.Yp, V, c->spec, (const float *)c->f[0],
+                                                           (const float *)c->f[1], (const float *)c->f[2], (const float *)c->f[3],
+                                                           c->d_A, c->d_rates, c->d_absorbed);
+    else
+        arc_finalize_kernel<double><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, c->p.Yp, V, c->spec, (const double *)c->f[0],
+                                                            (const double *)c->f[1], (const double *)c->f[2], (const double *)c->f[3],
+                                                            c->d_A, c->d_rates, c->d_absorbed);
+    return cudaGetLastError();
+}

@@ -1,0 +1,113 @@
+// arc_internal.cuh -- shared declarations of the CUDA path (not part of the public ABI).
+// Nothing here is shared with oracle/: both sides are typed from DESIGN.md's arithmetic contract.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include "../../include/arc.h"
+
+#define ARC_WARPS_PER_BLOCK 8
+#define ARC_TRACE_THREADS (32 * ARC_WARPS_PER_BLOCK)
+#define ARC_STACK_CAP 512            // families per warp-private stack: <= 32 per level
+#define ARC_QUEUE_CAP (1u << 16)     // families in the global donation queue
+#define ARC_BATCH_FAM 8              // families (x4 children = 32 rays) per warp batch
+
+// device-side error codes written to SchedState::error
+enum { ARC_DEV_OK = 0, ARC_DEV_STACK_OVERFLOW = 1, ARC_DEV_LOG_OVERFLOW = 2, ARC_DEV_WATCHDOG = 3, ARC_DEV_RAY_RUNAWAY = 4 };
+
+// A "family" = the 4 children 4*fam+j (j = 0..3) of one split (or 4 consecutive root pixels), all at
+// `level`, starting at the parent's split radius with the parent's optical depths.
+template <int NB>
+struct __align__(16) FamRec {
+    uint32_t src;
+    uint32_t fam;
+    uint32_t level;
+    uint32_t pad;
+    double tau[NB];
+};
+
+struct SchedState {
+    long long in_flight;                 // families alive anywhere, as known through flushes
+    unsigned long long seed_next;        // next unclaimed root family
+    unsigned long long q_head, q_tail;   // donation queue tickets (reserved pops / pushes)
+    int hungry;                          // warps idling for work
+    int error;                           // ARC_DEV_*
+    unsigned long long q_high;           // max(q_tail - q_head) seen
+    unsigned long long log_n;            // ray-log entries written
+};
+
+struct DevStats {
+    unsigned long long segments, rays, digest;
+    unsigned long long splits[ARC_MAX_LEVEL];
+    unsigned long long rays_level[ARC_MAX_LEVEL];
+    unsigned long long ends[3];
+    double escaped[ARC_MAX_BINS];
+    unsigned long long subcycles;
+    unsigned int max_sub;
+    unsigned int pad;
+};
+
+struct TraceArgs {
+    int N, nb, l0, Lmax, nsrc;
+    double dx;                 // cell size [cm]
+    double csplit;             // sqrt(3/(pi Phi)): split radius of level l = csplit * 2^l (cells)
+    double tau_term;
+    const void *kappa;         // [cell][nb] at field dtype
+    double *A;                 // [cell][nb] absorbed photons/s
+    const double *src_g;       // [nsrc][3] source position in grid units
+    const double *src_S;       // [nsrc][nb] Ndot * binfrac
+    unsigned char *stacks;     // n_warps * ARC_STACK_CAP family records
+    unsigned char *queue;      // ARC_QUEUE_CAP family records
+    unsigned long long *qseq;  // ARC_QUEUE_CAP slot sequence numbers
+    SchedState *sched;
+    DevStats *stats;
+    unsigned long long seed_total;  // nsrc * 3 * 4^l0
+    unsigned int fam_per_src;       // 3 * 4^l0
+    int seed_chunk;
+    // ray log (debug)
+    unsigned long long *log_key; unsigned int *log_seq; int *log_cell; unsigned long long log_cap;
+};
+
+struct Spectrum {
+    int nb;
+    double E[ARC_MAX_BINS];
+    double sig[3][ARC_MAX_BINS];
+};
+
+struct arc_ctx {
+    int N = 0, dtype = 0;
+    int64_t ncell = 0;
+    double box_cm = 0, dx = 0;
+    arc_params p;
+    cudaStream_t stream = 0;
+    void *f[5] = {0, 0, 0, 0, 0};     // n_H, x_HI, x_HeI, x_HeII, T at field dtype (SoA)
+    Spectrum spec;
+    bool have_fields = false, have_spec = false, have_src = false, have_rates = false;
+    int nsrc = 0;
+    double *d_src_g = 0, *d_src_S = 0;
+    double emitted[ARC_MAX_BINS];
+    void *d_kappa = 0; int kappa_nb = 0;
+    double *d_A = 0; int A_nb = 0;
+    double *d_rates = 0;              // 7 * ncell
+    unsigned char *d_stacks = 0; size_t stacks_bytes = 0;
+    unsigned char *d_queue = 0; unsigned long long *d_qseq = 0; size_t queue_bytes = 0;
+    SchedState *d_sched = 0;
+    DevStats *d_stats = 0;
+    double *d_absorbed = 0;           // [ARC_MAX_BINS] reduction scratch
+    int n_sm = 0;
+    int trace_grid = 0;
+    cudaEvent_t ev[8];                // 0..4: trace call (start, after opacity, after kernel, after finalize); 5,6: chemistry
+    bool traced_once = false, chem_once = false;
+    std::string err;
+};
+
+// arc_fields.cu
+cudaError_t arc_launch_opacity(arc_ctx *c);
+cudaError_t arc_launch_finalize(arc_ctx *c);
+// arc_trace.cu
+cudaError_t arc_launch_sched_reset(arc_ctx *c, unsigned long long seed_total);
+cudaError_t arc_launch_trace(arc_ctx *c, const TraceArgs &a, bool log, int *grid_out);
+int arc_trace_occupancy_grid(arc_ctx *c, int nb);
+cudaError_t arc_launch_pix2vec(const int32_t *d_level, const uint32_t *d_pix, int n, double *d_out, cudaStream_t s);
+// arc_chem.cu
+cudaError_t arc_launch_chemistry(arc_ctx *c, double dt);

@@ -1,0 +1,240 @@
+// arc_run.cu -- the compute entry points of include/arc.h: arc_trace, arc_update_chemistry, and the
+// read-back calls.  Launch order of one trace: scheduler reset -> a1+a2 opacity/zero ->
+// a3-a9 persistent tracer -> a10 finalize.  All on the context's stream; CUDA events bracket each kernel so
+// that callers (bench.py) can read per-kernel device times measured on the launching stream.
+#include "arc_internal.cuh"
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#define CK(call)                                                                                              \
+    do {                                                                                                      \
+        cudaError_t e_ = (call);                                                                              \
+        if (e_ != cudaSuccess) {                                                                              \
+            c->err = std::string(#call) + ": " + cudaGetErrorString(e_);                                      \
+            return e_ == cudaErrorMemoryAllocation ? ARC_ENOMEM : ARC_ECUDA;                                  \
+        }                                                                                                     \
+    } while (0)
+
+static int fail(arc_ctx *c, int code, const std::string &msg) { c->err = msg; return code; }
+
+static size_t famrec_bytes(int nb) { return (size_t)((16 + 8 * nb + 15) / 16) * 16; }
+
+// check the device-side error word after a synchronised trace
+static int device_error(arc_ctx *c)
+{
+    SchedState h;
+    CK(cudaMemcpy(&h, c->d_sched, sizeof(h), cudaMemcpyDeviceToHost));
+    if (h.error == ARC_DEV_OK && h.in_flight == 0) return ARC_OK;
+    c->have_rates = false;
+    switch (h.error) {
+        case ARC_DEV_STACK_OVERFLOW: return fail(c, ARC_EOVERFLOW, "arc_trace: a warp's work stack overflowed; rates are invalid");
+        case ARC_DEV_LOG_OVERFLOW: return fail(c, ARC_EOVERFLOW, "arc_trace_debug: ray log too small");
+        case ARC_DEV_WATCHDOG: return fail(c, ARC_ECUDA, "arc_trace: scheduler watchdog fired (no progress for 20 s); rates are invalid");
+        case ARC_DEV_RAY_RUNAWAY: return fail(c, ARC_ECUDA, "arc_trace: a ray exceeded 3N+8 segments; rates are invalid");
+        default: return fail(c, ARC_ECUDA, "arc_trace: kernel ended with work still in flight; rates are invalid");
+    }
+}
+
+static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, unsigned int *d_seq, int *d_cell)
+{
+    if (!c->have_fields) return fail(c, ARC_ESTATE, "arc_trace: no fields set (arc_set_fields)");
+    if (!c->have_spec) return fail(c, ARC_ESTATE, "arc_trace: no spectrum set (arc_set_spectrum)");
+    if (!c->have_src) return fail(c, ARC_ESTATE, "arc_trace: no sources set (arc_set_sources)");
+    const int nb = c->spec.nb;
+    // persistent grid: what is co-resident (SM count x blocks per SM), or the caller's override
+    const int resident = arc_trace_occupancy_grid(c, nb);
+    int grid = c->p.trace_blocks > 0 ? c->p.trace_blocks : resident;
+    if (grid > resident) grid = resident;         // blocks wait on one another: never oversubscribe
+    if (grid < 1) grid = 1;
+    c->trace_grid = grid;
+    const size_t rec = famrec_bytes(nb);
+    const size_t need_stacks = (size_t)grid * ARC_WARPS_PER_BLOCK * ARC_STACK_CAP * rec;
+    const size_t need_queue = (size_t)ARC_QUEUE_CAP * rec;
+    if (need_stacks > c->stacks_bytes) {
+        CK(cudaStreamSynchronize(c->stream));
+        cudaFree(c->d_stacks); c->d_stacks = nullptr; c->stacks_bytes = 0;
+        CK(cudaMalloc(&c->d_stacks, need_stacks));
+        c->stacks_bytes = need_stacks;
+    }
+    if (need_queue > c->queue_bytes) {
+        CK(cudaStreamSynchronize(c->stream));
+        cudaFree(c->d_queue); c->d_queue = nullptr; c->queue_bytes = 0;
+        CK(cudaMalloc(&c->d_queue, need_queue));
+        c->queue_bytes = need_queue;
+    }
+    if (!c->d_qseq) CK(cudaMalloc(&c->d_qseq, sizeof(unsigned long long) * ARC_QUEUE_CAP));
+
+    TraceArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.N = c->N; a.nb = nb; a.l0 = c->p.l0; a.Lmax = c->p.Lmax; a.nsrc = c->nsrc;
+    a.dx = c->dx;
+    a.csplit = std::sqrt(3.0 / (3.14159265358979323846 * c->p.Phi));      // O2: r_split(l) = csplit 2^l cells
+    a.tau_term = c->p.tau_term;
+    a.kappa = c->d_kappa; a.A = c->d_A; a.src_g = c->d_src_g; a.src_S = c->d_src_S;
+    a.stacks = c->d_stacks; a.queue = c->d_queue; a.qseq = c->d_qseq; a.sched = c->d_sched; a.stats = c->d_stats;
+    a.fam_per_src = 3u << (2 * c->p.l0);
+    a.seed_total = (unsigned long long)c->nsrc * a.fam_per_src;
+    a.seed_chunk = ARC_BATCH_FAM;
+    a.log_key = d_key; a.log_seq = d_seq; a.log_cell = d_cell; a.log_cap = log ? (unsigned long long)log->cap : 0ull;
+
+    CK(cudaEventRecord(c->ev[0], c->stream));
+    CK(arc_launch_sched_reset(c, a.seed_total));
+    CK(arc_launch_opacity(c));
+    CK(cudaEventRecord(c->ev[1], c->stream));
+    CK(arc_launch_trace(c, a, log != nullptr, nullptr));
+    CK(cudaEventRecord(c->ev[2], c->stream));
+    CK(arc_launch_finalize(c));
+    CK(cudaEventRecord(c->ev[3], c->stream));
+    c->traced_once = true;
+    c->have_rates = true;
+    if (!c->p.async || log) {
+        CK(cudaStreamSynchronize(c->stream));
+        return device_error(c);
+    }
+    return ARC_OK;
+}
+
+static void fill_rates(arc_ctx *c, arc_rates *out)
+{
+    const double *r = c->d_rates;
+    const int64_t n = c->ncell;
+    out->Gamma_HI = r; out->Gamma_HeI = r + n; out->Gamma_HeII = r + 2 * n;
+    out->heat_HI = r + 3 * n; out->heat_HeI = r + 4 * n; out->heat_HeII = r + 5 * n;
+    out->heat_total = r + 6 * n;
+}
+
+extern "C" {
+
+int arc_trace(arc_ctx *c, int step, arc_rates *out)
+{
+    (void)step;
+    if (!c) return ARC_EINVAL;
+    const int rc = run_trace(c, nullptr, nullptr, nullptr, nullptr);
+    if (rc == ARC_OK && out) fill_rates(c, out);
+    return rc;
+}
+
+int arc_trace_debug(arc_ctx *c, int step, arc_raylog *log)
+{
+    (void)step;
+    if (!c || !log) return ARC_EINVAL;
+    if (log->cap < 1 || !log->key || !log->seq || !log->cell) return fail(c, ARC_EINVAL, "arc_trace_debug: log buffers missing");
+    unsigned long long *d_key = nullptr; unsigned int *d_seq = nullptr; int *d_cell = nullptr;
+    log->n = 0;
+    cudaError_t e = cudaMalloc(&d_key, sizeof(unsigned long long) * log->cap);
+    if (e == cudaSuccess) e = cudaMalloc(&d_seq, sizeof(unsigned int) * log->cap);
+    if (e == cudaSuccess) e = cudaMalloc(&d_cell, sizeof(int) * log->cap);
+    int rc = ARC_OK;
+    if (e != cudaSuccess) { cudaGetLastError(); rc = fail(c, ARC_ENOMEM, "arc_trace_debug: cannot allocate the device log"); }
+    if (rc == ARC_OK) rc = run_trace(c, log, d_key, d_seq, d_cell);
+    if (rc == ARC_OK) {
+        SchedState h;
+        e = cudaMemcpy(&h, c->d_sched, sizeof(h), cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess) {
+            log->n = (int64_t)h.log_n;
+            if (h.log_n > (unsigned long long)log->cap) { c->have_rates = false; rc = fail(c, ARC_EOVERFLOW, "arc_trace_debug: ray log too small (log->n holds the size needed)"); }
+        }
+        if (e == cudaSuccess && rc == ARC_OK) e = cudaMemcpy(log->key, d_key, sizeof(unsigned long long) * log->n, cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess && rc == ARC_OK) e = cudaMemcpy(log->seq, d_seq, sizeof(unsigned int) * log->n, cudaMemcpyDeviceToHost);
+        if (e == cudaSuccess && rc == ARC_OK) e = cudaMemcpy(log->cell, d_cell, sizeof(int) * log->n, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) rc = fail(c, ARC_ECUDA, std::string("arc_trace_debug: ") + cudaGetErrorString(e));
+    }
+    cudaFree(d_key); cudaFree(d_seq); cudaFree(d_cell);
+    return rc;
+}
+
+int arc_get_rates(arc_ctx *c, double *Gamma_HI, double *Gamma_HeI, double *Gamma_HeII, double *heat_HI, double *heat_HeI,
+                  double *heat_HeII, double *heat_total, int where)
+{
+    if (!c) return ARC_EINVAL;
+    if (where != ARC_HOST && where != ARC_DEVICE) return fail(c, ARC_EINVAL, "arc_get_rates: bad `where`");
+    if (!c->have_rates) return fail(c, ARC_ESTATE, "arc_get_rates: no valid rates (call arc_trace)");
+    double *dst[7] = {Gamma_HI, Gamma_HeI, Gamma_HeII, heat_HI, heat_HeI, heat_HeII, heat_total};
+    const cudaMemcpyKind kind = (where == ARC_HOST) ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+    for (int i = 0; i < 7; ++i)
+        if (dst[i]) CK(cudaMemcpyAsync(dst[i], c->d_rates + (size_t)i * c->ncell, (size_t)c->ncell * sizeof(double), kind, c->stream));
+    if (where == ARC_HOST) CK(cudaStreamSynchronize(c->stream));
+    return ARC_OK;
+}
+
+int arc_get_accum(arc_ctx *c, double *A, int where)
+{
+    if (!c || !A) return ARC_EINVAL;
+    if (where != ARC_HOST && where != ARC_DEVICE) return fail(c, ARC_EINVAL, "arc_get_accum: bad `where`");
+    if (!c->have_rates) return fail(c, ARC_ESTATE, "arc_get_accum: no valid trace (call arc_trace)");
+    const cudaMemcpyKind kind = (where == ARC_HOST) ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+    CK(cudaMemcpyAsync(A, c->d_A, (size_t)c->ncell * c->spec.nb * sizeof(double), kind, c->stream));
+    if (where == ARC_HOST) CK(cudaStreamSynchronize(c->stream));
+    return ARC_OK;
+}
+
+int arc_update_chemistry(arc_ctx *c, double dt_s)
+{
+    if (!c) return ARC_EINVAL;
+    if (!(dt_s >= 0.0) || !std::isfinite(dt_s)) return fail(c, ARC_EINVAL, "arc_update_chemistry: dt must be finite and >= 0");
+    if (!c->have_rates) return fail(c, ARC_ESTATE, "arc_update_chemistry: no valid rates (call arc_trace after setting fields)");
+    CK(cudaEventRecord(c->ev[5], c->stream));
+    CK(cudaMemsetAsync(&c->d_stats->subcycles, 0, sizeof(unsigned long long) + 2 * sizeof(unsigned int), c->stream));
+    CK(arc_launch_chemistry(c, dt_s));
+    CK(cudaEventRecord(c->ev[6], c->stream));
+    c->chem_once = true;
+    // the rates stay valid as numbers, but they belong to the fields before this update
+    if (!c->p.async) CK(cudaStreamSynchronize(c->stream));
+    return ARC_OK;
+}
+
+int arc_synchronize(arc_ctx *c)
+{
+    if (!c) return ARC_EINVAL;
+    CK(cudaStreamSynchronize(c->stream));
+    if (c->traced_once) return device_error(c);
+    return ARC_OK;
+}
+
+int arc_get_stats(arc_ctx *c, arc_stats *s)
+{
+    if (!c || !s) return ARC_EINVAL;
+    std::memset(s, 0, sizeof(*s));
+    CK(cudaStreamSynchronize(c->stream));
+    DevStats d; SchedState h; double ab[ARC_MAX_BINS];
+    CK(cudaMemcpy(&d, c->d_stats, sizeof(d), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(&h, c->d_sched, sizeof(h), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(ab, c->d_absorbed, sizeof(ab), cudaMemcpyDeviceToHost));
+    s->segments = d.segments; s->rays = d.rays; s->digest = d.digest; s->queue_high_water = h.q_high;
+    for (int l = 0; l < ARC_MAX_LEVEL; ++l) { s->splits[l] = d.splits[l]; s->rays_level[l] = d.rays_level[l]; }
+    for (int i = 0; i < 3; ++i) s->ends[i] = d.ends[i];
+    for (int v = 0; v < ARC_MAX_BINS; ++v) { s->emitted[v] = c->have_src ? c->emitted[v] : 0.0; s->absorbed[v] = ab[v]; s->escaped[v] = d.escaped[v]; }
+    s->subcycles = d.subcycles; s->max_subcycles_cell = d.max_sub;
+    s->trace_grid = c->trace_grid;
+    if (c->traced_once) {
+        cudaEventElapsedTime(&s->trace_ms, c->ev[0], c->ev[3]);
+        cudaEventElapsedTime(&s->opacity_ms, c->ev[0], c->ev[1]);
+        cudaEventElapsedTime(&s->trace_kernel_ms, c->ev[1], c->ev[2]);
+        cudaEventElapsedTime(&s->finalize_ms, c->ev[2], c->ev[3]);
+    }
+    if (c->chem_once) cudaEventElapsedTime(&s->chem_ms, c->ev[5], c->ev[6]);
+    cudaGetLastError();
+    return ARC_OK;
+}
+
+int arc_pix2vec(const int32_t *level, const uint32_t *pix, int n, double *out)
+{
+    if (n < 0 || (n > 0 && (!level || !pix || !out))) return ARC_EINVAL;
+    if (n == 0) return ARC_OK;
+    for (int i = 0; i < n; ++i)
+        if (level[i] < 0 || level[i] > 14 || (unsigned long long)pix[i] >= (12ull << (2 * level[i]))) return ARC_EINVAL;
+    int32_t *d_l = nullptr; uint32_t *d_p = nullptr; double *d_o = nullptr;
+    cudaError_t e = cudaMalloc(&d_l, sizeof(int32_t) * n);
+    if (e == cudaSuccess) e = cudaMalloc(&d_p, sizeof(uint32_t) * n);
+    if (e == cudaSuccess) e = cudaMalloc(&d_o, sizeof(double) * 3 * n);
+    if (e == cudaSuccess) e = cudaMemcpy(d_l, level, sizeof(int32_t) * n, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(d_p, pix, sizeof(uint32_t) * n, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = arc_launch_pix2vec(d_l, d_p, n, d_o, 0);
+    if (e == cudaSuccess) e = cudaMemcpy(out, d_o, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost);
+    cudaFree(d_l); cudaFree(d_p); cudaFree(d_o);
+    if (e != cudaSuccess) { cudaGetLastError(); return ARC_ECUDA; }
+    return ARC_OK;
+}
+
+}  // extern "C"

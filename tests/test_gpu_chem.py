@@ -1,0 +1,119 @@
+"""GPU-vs-oracle parity of the per-cell update (a10 finalize + a11 chemistry) and of whole steps."""
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_1807_07094_b200 import arc, workloads as wl
+from gpu_common import RTOL, assert_close, compare_trace_stats
+
+pytestmark = pytest.mark.gpu
+
+
+def _fields_close(got, want, dtype, what=""):
+    names = ("n_H", "x_HI", "x_HeI", "x_HeII", "T")
+    for n, g, o in zip(names, got, want):
+        # fp32 storage: one rounding of the stored value on top of the 1e-3 bar is inside it
+        assert_close(g, o, RTOL[dtype], f"{what}{n}")
+
+
+@pytest.mark.parametrize("dtype,iso,Yp,nb", [("f64", 0, 0.24, 3), ("f32", 0, 0.24, 4), ("f64", 1, 0.0, 1), ("f32", 1, 0.24, 2)])
+def test_one_step_random_cells(dtype, iso, Yp, nb):
+    """random fields (x in 0.05..1, T in 1e2..3e4 K): trace on both sides, then chemistry on both sides"""
+    w = wl.tiny(N=12, nsrc=3, nb=nb, seed=61, dtype=dtype, Yp=Yp, kappa_scale=10.0)
+    w.params.update(isothermal=iso)
+    w.src_Ndot = w.src_Ndot * 1e3                      # strong enough to drive cells through many sub-cycles
+    ref = orc.step(w, w.fields())
+    with arc.Context(w, digest=1) as cx:
+        cx.trace()
+        st = cx.stats()
+        G, H, Ht = cx.rates()
+        cx.update_chemistry()
+        got = cx.get_fields()
+        st2 = cx.stats()
+    compare_trace_stats(st, ref["stats"], nb, RTOL[dtype])
+    assert_close(G, ref["Gamma"], RTOL[dtype], "Gamma")
+    assert_close(H, ref["heat"], RTOL[dtype], "heat")
+    _fields_close(got, ref["fields"], dtype)
+    # sub-cycle counts: decided by floating-point limiters, so equal up to a handful of cells
+    tot = int(ref["subcycles"].sum())
+    assert abs(st2["subcycles"] - tot) <= max(4, tot // 1000), (st2["subcycles"], tot)
+    assert st2["max_subcycles_cell"] >= 1
+
+
+def test_chemistry_with_injected_rates_matches_cell_by_cell():
+    """same rates on both sides (the GPU's), so only the update itself is compared"""
+    w = wl.tiny(N=10, nsrc=2, nb=3, seed=62, dtype="f64", kappa_scale=10.0)
+    w.src_Ndot = w.src_Ndot * 1e4
+    with arc.Context(w) as cx:
+        cx.trace()
+        G, H, _ = cx.rates()
+        cx.update_chemistry(w.dt_s * 3.0)
+        got = cx.get_fields()
+    want, sub = orc.chemistry(w, w.fields(), G, H, w.dt_s * 3.0)
+    _fields_close(got, want, "f64")
+    assert sub.max() > 1
+
+
+def test_subcycle_cap_is_honoured():
+    w = wl.tiny(N=6, nsrc=1, nb=2, seed=63, dtype="f64", kappa_scale=10.0)
+    w.src_Ndot = w.src_Ndot * 1e5
+    w.params.update(max_subcycles=3)
+    ref = orc.step(w, w.fields())
+    with arc.Context(w) as cx:
+        cx.trace(); cx.update_chemistry()
+        got = cx.get_fields(); st = cx.stats()
+    assert st["max_subcycles_cell"] <= 3
+    _fields_close(got, ref["fields"], "f64")
+
+
+def test_config1_ten_steps_with_oracle_fields_injected():
+    """SURVEY 8(c) parity protocol (ii): each step starts from the oracle's fields, so traversal (which
+    depends on depletion) is compared bit-exactly at every step; chemistry within tolerance."""
+    w = wl.config1()
+    fields = tuple(np.array(a, dtype=np.float64) for a in w.fields())
+    with arc.Context(w, digest=1) as cx:
+        for step in range(w.n_steps):
+            ref = orc.step(w, fields)
+            cx.set_fields(fields)
+            cx.trace(step)
+            st = cx.stats()
+            compare_trace_stats(st, ref["stats"], 1, RTOL["f64"])
+            assert_close(cx.accum(), ref["A"], RTOL["f64"], f"A step {step}")
+            cx.update_chemistry()
+            _fields_close(cx.get_fields(), ref["fields"], "f64", what=f"step {step} ")
+            fields = ref["fields"]
+
+
+def test_config1_free_running_ionized_volume_tracks_the_oracle():
+    """both sides evolve their own fields for 10 steps; compare the ionized volume (a physical integral)"""
+    w = wl.config1()
+    fields = tuple(np.array(a, dtype=np.float64) for a in w.fields())
+    with arc.Context(w) as cx:
+        for step in range(w.n_steps):
+            fields = orc.step(w, fields)["fields"]
+            cx.trace(step); cx.update_chemistry()
+        got = cx.get_fields()
+    vol_o = float((1.0 - fields[1]).sum()); vol_g = float((1.0 - got[1]).sum())
+    assert abs(vol_g - vol_o) <= 1e-6 * vol_o
+    assert_close(got[1], fields[1], 1e-4, "x_HI after 10 free-running steps", atol_frac=1e-9)
+
+
+def test_stromgren_growth_on_device():
+    """PAPER.md:255 Eq. 9 (sign per reading G1): r_I = r_S (1 - exp(-t/t_rec))^(1/3), uniform pure H,
+    T = 1e4 K, case B.  config 2 at 32^3 with small steps (front moves < 1 cell per step) - the same
+    run that pins the oracle in tests/test_oracle_chem.py."""
+    w = wl.config2(32)
+    t_rec = 1.0 / (wl.ALPHA_B_1E4 * 1e-3)
+    dt = 0.01 * t_rec
+    dx = w.box_cm / w.N
+    r_s = (3.0 * 5e48 / (4.0 * np.pi * wl.ALPHA_B_1E4 * 1e-6)) ** (1.0 / 3.0)
+    radii = []
+    with arc.Context(w) as cx:
+        for step in range(100):
+            cx.trace(step); cx.update_chemistry(dt)
+            if step % 10 == 9:
+                xe = (1.0 - cx.get_fields()[1] - 1.2e-3).clip(0)
+                radii.append((3.0 * float(xe.sum()) * dx ** 3 / (4.0 * np.pi)) ** (1.0 / 3.0))
+    assert np.all(np.diff(radii) > 0)
+    want = r_s * (1.0 - np.exp(-1.0)) ** (1.0 / 3.0)
+    assert abs(radii[-1] / want - 1.0) < 0.05, (radii[-1] / wl.KPC_CM, want / wl.KPC_CM)
