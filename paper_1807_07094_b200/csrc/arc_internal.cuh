@@ -9,7 +9,8 @@
 #define ARC_WARPS_PER_BLOCK 8
 #define ARC_TRACE_THREADS (32 * ARC_WARPS_PER_BLOCK)
 #define ARC_STACK_CAP 512            // families per warp-private stack: <= 32 per level
-#define ARC_QUEUE_CAP (1u << 16)     // families in the global donation queue
+#define ARC_QUEUE_CAP (1u << 18)     // ring slots of the global donation queue (>> warps x 32 + ARC_QUEUE_LOW)
+#define ARC_QUEUE_LOW 4096           // busy warps stop donating above this pool level
 #define ARC_BATCH_FAM 8              // families (x4 children = 32 rays) per warp batch
 
 // device-side error codes written to SchedState::error
@@ -30,6 +31,7 @@ struct SchedState {
     long long in_flight;                 // families alive anywhere, as known through flushes
     unsigned long long seed_next;        // next unclaimed root family
     unsigned long long q_head, q_tail;   // donation queue tickets (reserved pops / pushes)
+    long long q_count;                   // counting semaphore: published - claimed entries (may dip below 0)
     int hungry;                          // warps idling for work
     int error;                           // ARC_DEV_*
     unsigned long long q_high;           // max(q_tail - q_head) seen

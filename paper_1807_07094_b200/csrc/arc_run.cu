@@ -75,7 +75,10 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
     a.stacks = c->d_stacks; a.queue = c->d_queue; a.qseq = c->d_qseq; a.sched = c->d_sched; a.stats = c->d_stats;
     a.fam_per_src = 3u << (2 * c->p.l0);
     a.seed_total = (unsigned long long)c->nsrc * a.fam_per_src;
-    a.seed_chunk = ARC_BATCH_FAM;
+    {   // few sources: spread the root families over the warps instead of 8 per warp
+        const unsigned long long per_warp = a.seed_total / ((unsigned long long)grid * ARC_WARPS_PER_BLOCK);
+        a.seed_chunk = per_warp >= ARC_BATCH_FAM ? ARC_BATCH_FAM : (per_warp < 1 ? 1 : (int)per_warp);
+    }
     a.log_key = d_key; a.log_seq = d_seq; a.log_cell = d_cell; a.log_cap = log ? (unsigned long long)log->cap : 0ull;
 
     CK(cudaEventRecord(c->ev[0], c->stream));

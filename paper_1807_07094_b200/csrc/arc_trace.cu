@@ -111,14 +111,18 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, 2) arc_trace_kernel(const T
             if (delta != 0) { if (lane == 0) atomicAdd((unsigned long long *)&sc->in_flight, (unsigned long long)delta); delta = 0; }
             unsigned long long t_idle0 = 0; long long last_seen = 0; unsigned backoff = 64;
             for (;;) {
-                // (1) donated families
+                // (1) donated families: claim up to `want` published entries from the counting semaphore
+                // q_count, then take that many consecutive tickets.  No retry loops: every atomic succeeds.
                 int n = 0; unsigned long long ticket = 0;
                 if (lane == 0) {
-                    for (;;) {
-                        const unsigned long long h = ld_volatile_u64(&sc->q_head), t = ld_volatile_u64(&sc->q_tail);
-                        if (t <= h) break;
-                        const int want = (int)min((unsigned long long)ARC_BATCH_FAM, t - h);
-                        if (atomicCAS(&sc->q_head, h, h + want) == h) { n = want; ticket = h; break; }
+                    const long long avail = ld_volatile_s64(&sc->q_count);
+                    if (avail > 0) {
+                        const int hungry_now = max(ld_volatile_s32(&sc->hungry), 1);
+                        const long long want = max(1ll, min((long long)ARC_BATCH_FAM, avail / hungry_now));
+                        const long long before = (long long)atomicAdd((unsigned long long *)&sc->q_count, (unsigned long long)(-want));
+                        const long long got = max(0ll, min(before, want));
+                        if (got < want) atomicAdd((unsigned long long *)&sc->q_count, (unsigned long long)(want - got));
+                        if (got > 0) { ticket = atomicAdd(&sc->q_head, (unsigned long long)got); n = (int)got; }
                     }
                 }
                 n = __shfl_sync(0xffffffffu, n, 0);
@@ -336,27 +340,35 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, 2) arc_trace_kernel(const T
             int nd = (int)min((top - bot) / 2, 32u);
             unsigned long long ticket = 0;
             if (lane == 0) {
-                // flush first: donated families must be covered by the global counter before they are visible
-                if (delta != 0) atomicAdd((unsigned long long *)&sc->in_flight, (unsigned long long)delta);
-                for (;;) {
-                    const unsigned long long t = ld_volatile_u64(&sc->q_tail), hq = ld_volatile_u64(&sc->q_head);
-                    if (t - hq + nd > ARC_QUEUE_CAP) { nd = 0; break; }
-                    if (atomicCAS(&sc->q_tail, t, t + nd) == t) { ticket = t; atomicMax(&sc->q_high, t + nd - hq); break; }
+                // donate only while the pool is short of what the idle warps can take; the level test is
+                // approximate (plain loads), the ring is sized so that every warp overshooting at once still fits
+                const unsigned long long t = ld_volatile_u64(&sc->q_tail), hq = ld_volatile_u64(&sc->q_head);
+                const unsigned long long level_now = t > hq ? t - hq : 0ull;
+                if (level_now >= (unsigned long long)min(hungry * 4, ARC_QUEUE_LOW)) nd = 0;
+                else {
+                    // flush first: donated families must be covered by the global counter before they are visible
+                    if (delta != 0) atomicAdd((unsigned long long *)&sc->in_flight, (unsigned long long)delta);
+                    ticket = atomicAdd(&sc->q_tail, (unsigned long long)nd);
+                    atomicMax(&sc->q_high, ticket + nd - hq);
                 }
             }
-            delta = 0;
             nd = __shfl_sync(0xffffffffu, nd, 0);
             ticket = __shfl_sync(0xffffffffu, ticket, 0);
-            if (lane < nd) {
-                const unsigned long long tk = ticket + lane;
-                const unsigned slot = (unsigned)(tk % ARC_QUEUE_CAP);
-                while (ld_volatile_u64(&a.qseq[slot]) != tk) __nanosleep(32);    // previous lap's reader finished
-                const int4 *s4 = reinterpret_cast<const int4 *>(&STK(bot + lane));
-                int4 *d4 = reinterpret_cast<int4 *>(&queue[slot]);
+            if (nd > 0) {
+                delta = 0;
+                if (lane < nd) {
+                    const unsigned long long tk = ticket + lane;
+                    const unsigned slot = (unsigned)(tk % ARC_QUEUE_CAP);
+                    while (ld_volatile_u64(&a.qseq[slot]) != tk) __nanosleep(32);    // previous lap's reader finished
+                    const int4 *s4 = reinterpret_cast<const int4 *>(&STK(bot + lane));
+                    int4 *d4 = reinterpret_cast<int4 *>(&queue[slot]);
 #pragma unroll
-                for (int w = 0; w < (int)(sizeof(Rec) / 16); ++w) __stcg(d4 + w, s4[w]);
-                __threadfence();
-                *(volatile unsigned long long *)&a.qseq[slot] = tk + 1;            // publish
+                    for (int w = 0; w < (int)(sizeof(Rec) / 16); ++w) __stcg(d4 + w, s4[w]);
+                    __threadfence();
+                    *(volatile unsigned long long *)&a.qseq[slot] = tk + 1;            // publish
+                }
+                __syncwarp();
+                if (lane == 0) atomicAdd((unsigned long long *)&sc->q_count, (unsigned long long)nd);
             }
             bot += nd;
             __syncwarp();
@@ -425,7 +437,7 @@ __global__ void arc_sched_reset_kernel(SchedState *sc, DevStats *st, unsigned lo
     if (i < ARC_QUEUE_CAP) qseq[i] = i;
     if (i == 0) {
         sc->in_flight = (long long)seed_total; sc->seed_next = 0; sc->q_head = 0; sc->q_tail = 0;
-        sc->hungry = 0; sc->error = ARC_DEV_OK; sc->q_high = 0; sc->log_n = 0;
+        sc->hungry = 0; sc->error = ARC_DEV_OK; sc->q_high = 0; sc->log_n = 0; sc->q_count = 0;
         st->segments = 0; st->rays = 0; st->digest = 0;
         for (int l = 0; l < ARC_MAX_LEVEL; ++l) { st->splits[l] = 0; st->rays_level[l] = 0; }
         for (int e = 0; e < 3; ++e) st->ends[e] = 0;
