@@ -47,34 +47,70 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
     return t;
 }
 
-// opacity gather: one vector load per cell where the layout allows
+// opacity gather: the NB opacities of one cell, kept at their storage type until used (fewer registers while
+// the prefetched copy is in flight); one vector load per cell where the layout allows
+template <typename KT, int NB> struct KVec;
+template <int NB> struct KVec<float, NB> {
+    float k[NB];
+    __device__ __forceinline__ void load(const float *base, int cell)
+    {
+        const float *p = base + (long long)cell * NB;
+        if constexpr (NB % 4 == 0) {
+#pragma unroll
+            for (int v = 0; v < NB; v += 4) { const float4 q = __ldg((const float4 *)(p + v)); k[v] = q.x; k[v + 1] = q.y; k[v + 2] = q.z; k[v + 3] = q.w; }
+        } else if constexpr (NB % 2 == 0) {
+#pragma unroll
+            for (int v = 0; v < NB; v += 2) { const float2 q = __ldg((const float2 *)(p + v)); k[v] = q.x; k[v + 1] = q.y; }
+        } else {
+#pragma unroll
+            for (int v = 0; v < NB; ++v) k[v] = __ldg(p + v);
+        }
+    }
+    __device__ __forceinline__ double get(int v) const { return (double)k[v]; }
+};
+template <int NB> struct KVec<double, NB> {
+    double k[NB];
+    __device__ __forceinline__ void load(const double *base, int cell)
+    {
+        const double *p = base + (long long)cell * NB;
+        if constexpr (NB % 2 == 0) {
+#pragma unroll
+            for (int v = 0; v < NB; v += 2) { const double2 q = __ldg((const double2 *)(p + v)); k[v] = q.x; k[v + 1] = q.y; }
+        } else {
+#pragma unroll
+            for (int v = 0; v < NB; ++v) k[v] = __ldg(p + v);
+        }
+    }
+    __device__ __forceinline__ double get(int v) const { return k[v]; }
+};
 
-template <int NB>
-__device__ __forceinline__ void load_kappa(const float *k, long long cell, double (&out)[NB])
+// E = e^-x and ome = 1 - e^-x for x >= 0, both to ~2e-14 relative - ome also for tiny x, where 1 - E would
+// cancel.  Not a decision: terminations are decided on tau (sums and products only, contract C4).
+// x = -(k ln2 + r) with |r| <= ln2/2;  e^r - 1 = r q(r),  q(r) = sum_{n=0..10} r^n/(n+1)!
+__device__ __forceinline__ void arc_attenuate(double x, double &E, double &ome)
 {
-    const float *p = k + cell * NB;
-    if constexpr (NB == 4) { const float4 v = __ldg((const float4 *)p); out[0] = v.x; out[1] = v.y; out[2] = v.z; out[3] = v.w; }
-    else if constexpr (NB == 8) {
-        const float4 v = __ldg((const float4 *)p), w = __ldg((const float4 *)p + 1);
-        out[0] = v.x; out[1] = v.y; out[2] = v.z; out[3] = v.w; out[4] = w.x; out[5] = w.y; out[6] = w.z; out[7] = w.w;
-    }
-    else if constexpr (NB == 2) { const float2 v = __ldg((const float2 *)p); out[0] = v.x; out[1] = v.y; }
-    else {
-#pragma unroll
-        for (int v = 0; v < NB; ++v) out[v] = (double)__ldg(p + v);
-    }
-}
-template <int NB>
-__device__ __forceinline__ void load_kappa(const double *k, long long cell, double (&out)[NB])
-{
-    const double *p = k + cell * NB;
-    if constexpr (NB % 2 == 0) {
-#pragma unroll
-        for (int v = 0; v < NB; v += 2) { const double2 d = __ldg((const double2 *)(p + v)); out[v] = d.x; out[v + 1] = d.y; }
-    } else {
-#pragma unroll
-        for (int v = 0; v < NB; ++v) out[v] = __ldg(p + v);
-    }
+    const double MAGIC = 6755399441055744.0;                           // 1.5 * 2^52: round to nearest integer
+    const double kt = fma(x, -1.4426950408889634074, MAGIC);
+    const int k = __double2loint(kt);
+    const double kd = kt - MAGIC;
+    double r = fma(kd, -6.93147180369123816490e-01, -x);               // ln2 split in two parts
+    r = fma(kd, -1.90821492927058770002e-10, r);
+    double q = 1.0 / 39916800.0;
+    q = fma(q, r, 1.0 / 3628800.0);
+    q = fma(q, r, 1.0 / 362880.0);
+    q = fma(q, r, 1.0 / 40320.0);
+    q = fma(q, r, 1.0 / 5040.0);
+    q = fma(q, r, 1.0 / 720.0);
+    q = fma(q, r, 1.0 / 120.0);
+    q = fma(q, r, 1.0 / 24.0);
+    q = fma(q, r, 1.0 / 6.0);
+    q = fma(q, r, 0.5);
+    q = fma(q, r, 1.0);
+    const double em1 = r * q;                                          // e^r - 1
+    const double scale = __hiloint2double((max(k, -1022) + 1023) << 20, 0);    // 2^k
+    const double Ek = (x < 708.0) ? fma(em1, scale, scale) : 0.0;
+    E = Ek;
+    ome = (k == 0) ? -em1 : 1.0 - Ek;
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -195,7 +231,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, 2) arc_trace_kernel(const T
         double tau[NB], P[NB];
         double gx = 0, gy = 0, gz = 0, dirx = 0, diry = 0, dirz = 0, tx = 0, ty = 0, tz = 0, r = 0, r_end = 0;
         int ix = 0, iy = 0, iz = 0, sx = 0, sy = 0, sz = 0;
-        long long cell = 0;
+        int cell = 0;                          // N <= 1024: N^3 <= 2^30
         int end = -1;
         unsigned long long h = 0; unsigned int seq = 0;
         if (active) {
@@ -227,7 +263,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, 2) arc_trace_kernel(const T
                 end = ARC_END_ESCAPED; active = false;
             } else {
                 ix = (int)fx; iy = (int)fy; iz = (int)fz;
-                cell = ((long long)iz * N + iy) * N + ix;
+                cell = (iz * N + iy) * N + ix;
                 sx = dirx > 0.0 ? 1 : (dirx < 0.0 ? -1 : 0);
                 sy = diry > 0.0 ? 1 : (diry < 0.0 ? -1 : 0);
                 sz = dirz > 0.0 ? 1 : (dirz < 0.0 ? -1 : 0);
@@ -239,32 +275,46 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, 2) arc_trace_kernel(const T
         }
 
         // ------------------------------------------------------------------ a6/a7: the segment loop
+        // One iteration = one (ray, cell) segment.  The axis advance is branch-free (one IEEE division per
+        // segment, whichever axis is crossed) and the next cell's opacities are requested BEFORE this segment's
+        // attenuation arithmetic, so the gather latency hides behind it.
         const unsigned int max_seg = 3u * (unsigned)N + 8u;
         unsigned int nray_seg = 0;
+        KVec<KT, NB> kcur;
+        if (active) kcur.load(kappa, cell);
         while (active) {
             int ax = 0; double tmin = tx;
             if (ty < tmin) { tmin = ty; ax = 1; }
             if (tz < tmin) { tmin = tz; ax = 2; }
             const bool split = (r_end <= tmin);
             const double r_out = split ? r_end : tmin;
-            double ds = arc_sub(r_out, r);
-            if (ds < 0.0) ds = 0.0;
-            const double dl = arc_mul(ds, a.dx);
-            double kap[NB];
-            load_kappa<NB>(kappa, cell, kap);
+            const double dl = arc_mul(fmax(arc_sub(r_out, r), 0.0), a.dx);
+            // a6: where the ray goes next (used only if it neither splits nor ends here)
+            const int st = ax == 0 ? sx : (ax == 1 ? sy : sz);
+            const int inext = (ax == 0 ? ix : (ax == 1 ? iy : iz)) + st;
+            const bool out = (unsigned)inext >= (unsigned)N;
+            const int stride = ax == 0 ? 1 : (ax == 1 ? N : N * N);
+            const int cell_next = cell + st * stride;
+            KVec<KT, NB> knext;
+            if (!split && !out) knext.load(kappa, cell_next);
+            const double g_ax = ax == 0 ? gx : (ax == 1 ? gy : gz);
+            const double d_ax = ax == 0 ? dirx : (ax == 1 ? diry : dirz);
+            const double t_new = __ddiv_rn(arc_sub((double)(inext + (st > 0)), g_ax), d_ax);
+            // a7: optical depth and deposit (Eq. 1)
             double av[NB];
             double taumin = __longlong_as_double(0x7ff0000000000000ll);
 #pragma unroll
             for (int v = 0; v < NB; ++v) {
-                const double dtau = arc_mul(kap[v], dl);
+                const double dtau = arc_mul(kcur.get(v), dl);
                 tau[v] = arc_add(tau[v], dtau);                 // decides termination: IEEE, no FMA (C4)
                 taumin = fmin(taumin, tau[v]);
-                const double em = expm1(-dtau);                 // Eq. 1: absorbed = P (1 - e^-dtau)
-                av[v] = -P[v] * em;
-                P[v] = fma(P[v], em, P[v]);                     // photon conserving: P <- P e^-dtau
+                double E, ome;
+                arc_attenuate(dtau, E, ome);                    // e^-dtau and 1 - e^-dtau
+                av[v] = P[v] * ome;                             // absorbed = P (1 - e^-dtau)
+                P[v] = P[v] * E;                                // photon conserving: the ray keeps P e^-dtau
             }
             const bool depleted = (taumin >= a.tau_term);
-            double *Ac = a.A + cell * NB;
+            double *Ac = a.A + (long long)cell * NB;
 #pragma unroll
             for (int v = 0; v < NB; ++v) {
                 if (depleted) av[v] += P[v];                    // reading G7: the remainder stays in this cell
@@ -276,23 +326,20 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, 2) arc_trace_kernel(const T
                 const unsigned long long e = atomicAdd(&sc->log_n, 1ull);
                 if (e < a.log_cap) {
                     a.log_key[e] = ((unsigned long long)src << 40) | ((unsigned long long)level << 32) | pix;
-                    a.log_seq[e] = seq; a.log_cell[e] = (int)cell;
+                    a.log_seq[e] = seq; a.log_cell[e] = cell;
                 }
                 ++seq;
             }
-            r = r_out;
             if (depleted) { end = ARC_END_DEPLETED; active = false; }
             else if (split) { end = ARC_END_SPLIT; active = false; }
-            else {
-                bool out;
-                if (ax == 0) { ix += sx; out = (unsigned)ix >= (unsigned)N; cell += sx; tx = __ddiv_rn(arc_sub((double)(ix + (sx > 0)), gx), dirx); }
-                else if (ax == 1) { iy += sy; out = (unsigned)iy >= (unsigned)N; cell += (long long)sy * N; ty = __ddiv_rn(arc_sub((double)(iy + (sy > 0)), gy), diry); }
-                else { iz += sz; out = (unsigned)iz >= (unsigned)N; cell += (long long)sz * N * N; tz = __ddiv_rn(arc_sub((double)(iz + (sz > 0)), gz), dirz); }
-                if (out) {
+            else if (out) {
 #pragma unroll
-                    for (int v = 0; v < NB; ++v) atomicAdd(&s_esc[v], P[v]);
-                    end = ARC_END_ESCAPED; active = false;
-                } else if (nray_seg > max_seg) { atomicCAS(&sc->error, 0, ARC_DEV_RAY_RUNAWAY); end = ARC_END_ESCAPED; active = false; }
+                for (int v = 0; v < NB; ++v) atomicAdd(&s_esc[v], P[v]);
+                end = ARC_END_ESCAPED; active = false;
+            } else if (nray_seg > max_seg) { atomicCAS(&sc->error, 0, ARC_DEV_RAY_RUNAWAY); end = ARC_END_ESCAPED; active = false; }
+            else {
+                r = r_out; cell = cell_next; kcur = knext;
+                if (ax == 0) { ix = inext; tx = t_new; } else if (ax == 1) { iy = inext; ty = t_new; } else { iz = inext; tz = t_new; }
             }
         }
         __syncwarp();
