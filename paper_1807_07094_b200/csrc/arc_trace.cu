@@ -47,6 +47,13 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
     return t;
 }
 
+// fire-and-forget fp64 reduction (REDG.E.ADD.F64): written as PTX `red` because ptxas otherwise emits the returning
+// form (ATOMG ... RZ) inside this kernel's divergent loop, which holds a scoreboard until L2 answers
+__device__ __forceinline__ void arc_red_add(double *p, double v)
+{
+    asm volatile("red.relaxed.gpu.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
+}
+
 // opacity gather: the NB opacities of one cell, kept at their storage type until used (fewer registers while
 // the prefetched copy is in flight); one vector load per cell where the layout allows
 template <typename KT, int NB> struct KVec;
@@ -318,7 +325,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, 2) arc_trace_kernel(const T
 #pragma unroll
             for (int v = 0; v < NB; ++v) {
                 if (depleted) av[v] += P[v];                    // reading G7: the remainder stays in this cell
-                atomicAdd(Ac + v, av[v]);                       // a7: RED.ADD.F64 ("atomically")
+                arc_red_add(Ac + v, av[v]);                     // a7: RED.ADD.F64 ("atomically")
             }
             ++nseg; ++nray_seg;
             if (FLAGS & FLAG_DIGEST) h = mix64(h ^ (unsigned long long)cell);
