@@ -180,9 +180,10 @@ def run_cuda(args):
 
     # ---- arm 1: inputs resident in HBM (device tensors handed over once, before the timed region)
     dev_fields = [torch.from_numpy(np.ascontiguousarray(np.asarray(a, dtype=fdt))).cuda() for a in w.fields()]
-    cx = arc.Context(w, fields=dev_fields, stream=stream.cuda_stream)
+    extra = {"deposit": args.deposit} if args.deposit else {}
+    cx = arc.Context(w, fields=dev_fields, stream=stream.cuda_stream, **extra)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    seg_steps, kern_ms, chem_ms, trace_ms, sub_steps = [], [], [], [], []
+    seg_steps, kern_ms, chem_ms, trace_ms, sub_steps, rec_steps = [], [], [], [], [], []
 
     def one_step(i, record):
         cx.trace(i)
@@ -190,7 +191,7 @@ def run_cuda(args):
         if record:
             st = cx.stats()                       # synchronises the stream; reads the per-kernel event times
             seg_steps.append(st["segments"]); kern_ms.append(st["trace_kernel_ms"]); chem_ms.append(st["chem_ms"])
-            trace_ms.append(st["trace_ms"]); sub_steps.append(st["subcycles"])
+            trace_ms.append(st["trace_ms"]); sub_steps.append(st["subcycles"]); rec_steps.append(st["deposit_records"])
 
     for i in range(args.warmup):
         one_step(i, False)
@@ -215,7 +216,7 @@ def run_cuda(args):
     # ---- arm 2: end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     pin = [torch.from_numpy(np.ascontiguousarray(np.asarray(a, dtype=fdt))).pin_memory() for a in w.fields()]
     rates_host = [torch.empty(nc, dtype=torch.float64).pin_memory() for _ in range(4)]   # Gamma_HI, Gamma_HeI, Gamma_HeII, heat_total
-    cx2 = arc.Context(w, fields=[p.numpy() for p in pin], stream=stream.cuda_stream)
+    cx2 = arc.Context(w, fields=[p.numpy() for p in pin], stream=stream.cuda_stream, **extra)
     h2d = 5 * nc * pin[0].element_size()
     d2h = 4 * nc * pin[0].element_size() + 4 * nc * 8
     e2e_seg = 0
@@ -263,7 +264,7 @@ def run_cuda(args):
             "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, paper_1807_07094_b200/workloads.py)",
             "config": dict(describe(w), parallelism="replicas" if world > 1 else "single-gpu",
                            l2_policy="inputs larger than L2" if (nc * nb * (bytes_seg // nb)) > 126e6 else "working set fits L2 (small config)",
-                           trace_grid_blocks=trace_grid),
+                           trace_grid_blocks=trace_grid, deposit=args.deposit),
             "e2e": {"value": e2e_seg_all / (e2e_ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": 5 * args.steps,
             "clocks": clocks,
@@ -277,6 +278,7 @@ def run_cuda(args):
             "cell_updates_per_s": nc * args.steps / (sum(chem_ms) * 1e-3) if sum(chem_ms) > 0 else 0.0,
             "chem_subcycles_per_step": [int(x) for x in sub_steps],
             "photon_conservation_max_rel_err": conservation,
+            "segments_per_deposit_record": tot_seg / max(1.0, float(sum(rec_steps))),
             "host_wall_s": wall,
         }
         if world == 1 and not args.no_cpu_baseline:
@@ -297,6 +299,7 @@ def main():
     ap.add_argument("--config", default="config4")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--deposit", type=int, default=0, help="arc_params.deposit: 0 auto, 1 per-lane REDs, 2 warp-aggregated")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -20,6 +20,7 @@ ARC_F32, ARC_F64 = 0, 1
 ARC_HOST, ARC_DEVICE = 0, 1
 ARC_OK, ARC_EINVAL, ARC_ENOMEM, ARC_ECUDA, ARC_ESTATE, ARC_EOVERFLOW = 0, -1, -2, -3, -4, -5
 ARC_END_SPLIT, ARC_END_DEPLETED, ARC_END_ESCAPED = 0, 1, 2
+ARC_DEPOSIT_AUTO, ARC_DEPOSIT_RED, ARC_DEPOSIT_AGG = 0, 1, 2
 ARC_MAX_BINS, ARC_MAX_LEVEL = 8, 16
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -41,7 +42,7 @@ class arc_params(C.Structure):
     _fields_ = [("l0", C.c_int32), ("Lmax", C.c_int32), ("Phi", C.c_double), ("tau_term", C.c_double),
                 ("Yp", C.c_double), ("isothermal", C.c_int32), ("caseB", C.c_int32), ("coll_ion", C.c_int32),
                 ("max_subcycles", C.c_int32), ("eps_sub", C.c_double), ("x_floor", C.c_double),
-                ("digest", C.c_int32), ("async_", C.c_int32), ("trace_blocks", C.c_int32), ("reserved", C.c_int32)]
+                ("digest", C.c_int32), ("async_", C.c_int32), ("trace_blocks", C.c_int32), ("deposit", C.c_int32)]
 
 
 class arc_rates(C.Structure):
@@ -57,7 +58,8 @@ class arc_stats(C.Structure):
                 ("escaped", C.c_double * ARC_MAX_BINS), ("subcycles", C.c_uint64),
                 ("max_subcycles_cell", C.c_uint32), ("pad", C.c_uint32), ("trace_ms", C.c_float),
                 ("chem_ms", C.c_float), ("trace_kernel_ms", C.c_float), ("opacity_ms", C.c_float),
-                ("finalize_ms", C.c_float), ("trace_grid", C.c_int32)]
+                ("finalize_ms", C.c_float), ("trace_grid", C.c_int32), ("pad2", C.c_int32),
+                ("deposit_records", C.c_uint64)]
 
 
 class arc_raylog(C.Structure):
@@ -249,7 +251,8 @@ def stats_dict(s: arc_stats, nb: int) -> dict:
                 absorbed=np.array(s.absorbed[:nb]), escaped=np.array(s.escaped[:nb]),
                 subcycles=int(s.subcycles), max_subcycles_cell=int(s.max_subcycles_cell),
                 trace_ms=float(s.trace_ms), chem_ms=float(s.chem_ms), trace_kernel_ms=float(s.trace_kernel_ms),
-                opacity_ms=float(s.opacity_ms), finalize_ms=float(s.finalize_ms), trace_grid=int(s.trace_grid))
+                opacity_ms=float(s.opacity_ms), finalize_ms=float(s.finalize_ms), trace_grid=int(s.trace_grid),
+                deposit_records=int(s.deposit_records))
 
 
 def params_from_dict(d: dict, **override) -> arc_params:

@@ -37,7 +37,7 @@ void arc_default_params(arc_params *p)
     std::memset(p, 0, sizeof(*p));
     p->l0 = 1; p->Lmax = 13; p->Phi = 3.0; p->tau_term = 30.0; p->Yp = 0.0;
     p->isothermal = 1; p->caseB = 1; p->coll_ion = 0; p->max_subcycles = 4096;
-    p->eps_sub = 0.1; p->x_floor = 1e-12; p->digest = 0; p->async = 0; p->trace_blocks = 0;
+    p->eps_sub = 0.1; p->x_floor = 1e-12; p->digest = 0; p->async = 0; p->trace_blocks = 0; p->deposit = ARC_DEPOSIT_AUTO;
 }
 
 int arc_create_grid(arc_ctx **out, int N, double box_cm, int dtype)
@@ -111,6 +111,7 @@ int arc_set_params(arc_ctx *c, const arc_params *p)
     if (!(p->eps_sub > 0.0)) return fail(c, ARC_EINVAL, "arc_set_params: eps_sub must be positive");
     if (!(p->x_floor >= 0.0 && p->x_floor < 1.0)) return fail(c, ARC_EINVAL, "arc_set_params: x_floor must be in [0, 1)");
     if (p->trace_blocks < 0) return fail(c, ARC_EINVAL, "arc_set_params: trace_blocks must be >= 0");
+    if (p->deposit < ARC_DEPOSIT_AUTO || p->deposit > ARC_DEPOSIT_AGG) return fail(c, ARC_EINVAL, "arc_set_params: bad deposit mode");
     c->p = *p;
     c->have_rates = false;
     return ARC_OK;
@@ -166,7 +167,7 @@ int arc_set_spectrum(arc_ctx *c, int nbins, const double *E_eV, const double *si
     if (nbins != c->spec.nb || !c->d_kappa) {
         cudaFree(c->d_kappa); cudaFree(c->d_A); c->d_kappa = nullptr; c->d_A = nullptr;
         CK(cudaMalloc(&c->d_kappa, (size_t)c->ncell * nbins * esize(c)));
-        CK(cudaMalloc(&c->d_A, (size_t)c->ncell * nbins * sizeof(double)));
+        CK(cudaMalloc(&c->d_A, (size_t)c->ncell * arc_nbp(nbins) * sizeof(double)));
         if (c->have_src && nbins != c->spec.nb) c->have_src = false;      // binfrac rows no longer match
     }
     std::memset(&c->spec, 0, sizeof(c->spec));

@@ -12,7 +12,7 @@ namespace {
 __device__ __forceinline__ double n_helium(double nH, double Yp) { return nH * Yp / (4.0 * (1.0 - Yp)); }
 
 template <typename FT>
-__global__ void __launch_bounds__(256) arc_opacity_kernel(long long ncell, int nb, double Yp, Spectrum sp,
+__global__ void __launch_bounds__(256) arc_opacity_kernel(long long ncell, int nb, int nbp, double Yp, Spectrum sp,
                                                          const FT *__restrict__ nH, const FT *__restrict__ xHI,
                                                          const FT *__restrict__ xHeI, const FT *__restrict__ xHeII,
                                                          FT *__restrict__ kappa, double *__restrict__ A)
@@ -27,13 +27,13 @@ __global__ void __launch_bounds__(256) arc_opacity_kernel(long long ncell, int n
             const double k = __dadd_rn(__dadd_rn(__dmul_rn(sp.sig[0][v], nHI), __dmul_rn(sp.sig[1][v], nHeI)),
                                        __dmul_rn(sp.sig[2][v], nHeII));
             kappa[c * nb + v] = (FT)k;
-            A[c * nb + v] = 0.0;
         }
+        for (int v = 0; v < nbp; ++v) A[c * nbp + v] = 0.0;
     }
 }
 
 template <typename FT>
-__global__ void __launch_bounds__(256) arc_finalize_kernel(long long ncell, int nb, double Yp, double V, Spectrum sp,
+__global__ void __launch_bounds__(256) arc_finalize_kernel(long long ncell, int nb, int nbp, double Yp, double V, Spectrum sp,
                                                           const FT *__restrict__ nH, const FT *__restrict__ xHI,
                                                           const FT *__restrict__ xHeI, const FT *__restrict__ xHeII,
                                                           const double *__restrict__ A, double *__restrict__ rates,
@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(256) arc_finalize_kernel(long long ncell, int 
 #pragma unroll
         for (int v = 0; v < ARC_MAX_BINS; ++v) {
             if (v >= nb) break;
-            const double Av = A[c * nb + v];
+            const double Av = A[c * nbp + v];
             acc[v] += Av;
             const double kp = (sp.sig[0][v] * ns[0] + sp.sig[1][v] * ns[1]) + sp.sig[2][v] * ns[2];
             if (kp > 0.0) {
@@ -99,11 +99,11 @@ cudaError_t arc_launch_opacity(arc_ctx *c)
 {
     const int g = stream_grid(c, c->ncell);
     if (c->dtype == ARC_F32)
-        arc_opacity_kernel<float><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, c->p.Yp, c->spec, (const float *)c->f[0],
+        arc_opacity_kernel<float><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, arc_nbp(c->spec.nb), c->p.Yp, c->spec, (const float *)c->f[0],
                                                           (const float *)c->f[1], (const float *)c->f[2], (const float *)c->f[3],
                                                           (float *)c->d_kappa, c->d_A);
     else
-        arc_opacity_kernel<double><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, c->p.Yp, c->spec, (const double *)c->f[0],
+        arc_opacity_kernel<double><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, arc_nbp(c->spec.nb), c->p.Yp, c->spec, (const double *)c->f[0],
                                                            (const double *)c->f[1], (const double *)c->f[2], (const double *)c->f[3],
                                                            (double *)c->d_kappa, c->d_A);
     return cudaGetLastError();
@@ -116,11 +116,11 @@ cudaError_t arc_launch_finalize(arc_ctx *c)
     const int g = stream_grid(c, c->ncell);
     const double V = c->dx * c->dx * c->dx;
     if (c->dtype == ARC_F32)
-        arc_finalize_kernel<float><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, c->p.Yp, V, c->spec, (const float *)c->f[0],
+        arc_finalize_kernel<float><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, arc_nbp(c->spec.nb), c->p.Yp, V, c->spec, (const float *)c->f[0],
                                                            (const float *)c->f[1], (const float *)c->f[2], (const float *)c->f[3],
                                                            c->d_A, c->d_rates, c->d_absorbed);
     else
-        arc_finalize_kernel<double><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, c->p.Yp, V, c->spec, (const double *)c->f[0],
+        arc_finalize_kernel<double><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, arc_nbp(c->spec.nb), c->p.Yp, V, c->spec, (const double *)c->f[0],
                                                             (const double *)c->f[1], (const double *)c->f[2], (const double *)c->f[3],
                                                             c->d_A, c->d_rates, c->d_absorbed);
     return cudaGetLastError();

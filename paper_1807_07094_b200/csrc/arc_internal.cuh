@@ -39,7 +39,7 @@ struct SchedState {
 };
 
 struct DevStats {
-    unsigned long long segments, rays, digest;
+    unsigned long long segments, rays, digest, deposit_records;
     unsigned long long splits[ARC_MAX_LEVEL];
     unsigned long long rays_level[ARC_MAX_LEVEL];
     unsigned long long ends[3];
@@ -49,13 +49,18 @@ struct DevStats {
     unsigned int pad;
 };
 
+// stride (in doubles) of one cell's accumulators: nb rounded up to even (nb > 1) so that a cell's record is a
+// multiple of 16 bytes, 16-byte aligned - the granule of cp.reduce.async.bulk
+static inline int arc_nbp(int nb) { return nb == 1 ? 1 : ((nb + 1) & ~1); }
+
 struct TraceArgs {
     int N, nb, l0, Lmax, nsrc;
+    int nbp;                   // accumulator stride, arc_nbp(nb)
     double dx;                 // cell size [cm]
     double csplit;             // sqrt(3/(pi Phi)): split radius of level l = csplit * 2^l (cells)
     double tau_term;
     const void *kappa;         // [cell][nb] at field dtype
-    double *A;                 // [cell][nb] absorbed photons/s
+    double *A;                 // [cell][nbp] absorbed photons/s (entries nb..nbp-1 stay zero)
     const double *src_g;       // [nsrc][3] source position in grid units
     const double *src_S;       // [nsrc][nb] Ndot * binfrac
     unsigned char *stacks;     // n_warps * ARC_STACK_CAP family records
@@ -66,6 +71,7 @@ struct TraceArgs {
     unsigned long long seed_total;  // nsrc * 3 * 4^l0
     unsigned int fam_per_src;       // 3 * 4^l0
     int seed_chunk;
+    int flags;                      // kernel variant: 1 = per-ray log, 2 = traversal digest
     // ray log (debug)
     unsigned long long *log_key; unsigned int *log_seq; int *log_cell; unsigned long long log_cap;
 };
@@ -109,7 +115,7 @@ cudaError_t arc_launch_finalize(arc_ctx *c);
 // arc_trace.cu
 cudaError_t arc_launch_sched_reset(arc_ctx *c, unsigned long long seed_total);
 cudaError_t arc_launch_trace(arc_ctx *c, const TraceArgs &a, bool log, int *grid_out);
-int arc_trace_occupancy_grid(arc_ctx *c, int nb);
+int arc_trace_occupancy_grid(arc_ctx *c, int nb, int flags);   // flags: 1 log, 2 digest
 cudaError_t arc_launch_pix2vec(const int32_t *d_level, const uint32_t *d_pix, int n, double *d_out, cudaStream_t s);
 // arc_chem.cu
 cudaError_t arc_launch_chemistry(arc_ctx *c, double dt);

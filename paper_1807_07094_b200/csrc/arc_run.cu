@@ -43,7 +43,8 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
     if (!c->have_src) return fail(c, ARC_ESTATE, "arc_trace: no sources set (arc_set_sources)");
     const int nb = c->spec.nb;
     // persistent grid: what is co-resident (SM count x blocks per SM), or the caller's override
-    const int resident = arc_trace_occupancy_grid(c, nb);
+    const int flags = log ? 3 : (c->p.digest ? 2 : 0);
+    const int resident = arc_trace_occupancy_grid(c, nb, flags);
     int grid = c->p.trace_blocks > 0 ? c->p.trace_blocks : resident;
     if (grid > resident) grid = resident;         // blocks wait on one another: never oversubscribe
     if (grid < 1) grid = 1;
@@ -67,7 +68,7 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
 
     TraceArgs a;
     std::memset(&a, 0, sizeof(a));
-    a.N = c->N; a.nb = nb; a.l0 = c->p.l0; a.Lmax = c->p.Lmax; a.nsrc = c->nsrc;
+    a.N = c->N; a.nb = nb; a.nbp = arc_nbp(nb); a.l0 = c->p.l0; a.Lmax = c->p.Lmax; a.nsrc = c->nsrc;
     a.dx = c->dx;
     a.csplit = std::sqrt(3.0 / (3.14159265358979323846 * c->p.Phi));      // O2: r_split(l) = csplit 2^l cells
     a.tau_term = c->p.tau_term;
@@ -79,6 +80,7 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
         const unsigned long long per_warp = a.seed_total / ((unsigned long long)grid * ARC_WARPS_PER_BLOCK);
         a.seed_chunk = per_warp >= ARC_BATCH_FAM ? ARC_BATCH_FAM : (per_warp < 1 ? 1 : (int)per_warp);
     }
+    a.flags = flags;
     a.log_key = d_key; a.log_seq = d_seq; a.log_cell = d_cell; a.log_cap = log ? (unsigned long long)log->cap : 0ull;
 
     CK(cudaEventRecord(c->ev[0], c->stream));
@@ -167,7 +169,9 @@ int arc_get_accum(arc_ctx *c, double *A, int where)
     if (where != ARC_HOST && where != ARC_DEVICE) return fail(c, ARC_EINVAL, "arc_get_accum: bad `where`");
     if (!c->have_rates) return fail(c, ARC_ESTATE, "arc_get_accum: no valid trace (call arc_trace)");
     const cudaMemcpyKind kind = (where == ARC_HOST) ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
-    CK(cudaMemcpyAsync(A, c->d_A, (size_t)c->ncell * c->spec.nb * sizeof(double), kind, c->stream));
+    const int nb = c->spec.nb, nbp = arc_nbp(nb);        // device rows are padded to nbp doubles; the caller gets [cell][nb]
+    if (nbp == nb) CK(cudaMemcpyAsync(A, c->d_A, (size_t)c->ncell * nb * sizeof(double), kind, c->stream));
+    else CK(cudaMemcpy2DAsync(A, nb * sizeof(double), c->d_A, nbp * sizeof(double), nb * sizeof(double), (size_t)c->ncell, kind, c->stream));
     if (where == ARC_HOST) CK(cudaStreamSynchronize(c->stream));
     return ARC_OK;
 }
@@ -204,7 +208,7 @@ int arc_get_stats(arc_ctx *c, arc_stats *s)
     CK(cudaMemcpy(&d, c->d_stats, sizeof(d), cudaMemcpyDeviceToHost));
     CK(cudaMemcpy(&h, c->d_sched, sizeof(h), cudaMemcpyDeviceToHost));
     CK(cudaMemcpy(ab, c->d_absorbed, sizeof(ab), cudaMemcpyDeviceToHost));
-    s->segments = d.segments; s->rays = d.rays; s->digest = d.digest; s->queue_high_water = h.q_high;
+    s->deposit_records = d.deposit_records; s->segments = d.segments; s->rays = d.rays; s->digest = d.digest; s->queue_high_water = h.q_high;
     for (int l = 0; l < ARC_MAX_LEVEL; ++l) { s->splits[l] = d.splits[l]; s->rays_level[l] = d.rays_level[l]; }
     for (int i = 0; i < 3; ++i) s->ends[i] = d.ends[i];
     for (int v = 0; v < ARC_MAX_BINS; ++v) { s->emitted[v] = c->have_src ? c->emitted[v] : 0.0; s->absorbed[v] = ab[v]; s->escaped[v] = d.escaped[v]; }

@@ -1,0 +1,611 @@
+// arc_trace_kernel.cuh -- the persistent ray-tracing kernel, as a template that the
+// arc_trace_inst_*.cu translation units instantiate (split so that they compile in parallel).
+//
+// What it computes (Eq. 1; O1-O3): every source emits 12*4^l0 HEALPix
+// rays; a ray marches cell by cell (3D-DDA: next X, Y or Z boundary), each segment adds
+// S_nu e^-tau_nu (1 - e^-dtau_nu) absorbed photons/s to the cell's accumulator (atomically),
+// and at radius r_split(l) = sqrt(3/(pi Phi)) 2^l cells the ray is replaced by its 4 HEALPix children.
+//
+// How (B200 design, NOT the paper's per-source, per-level launches - PAPER.md:49-54 is prior art):
+//  * ONE launch for all sources and all levels.  The grid is sized to what is co-resident
+//    (SMs x blocks/SM); every warp runs a work loop until a global in-flight counter reaches zero.
+//  * Work item = a FAMILY (4 sibling rays sharing start radius and optical depths), so a split costs one
+//    record; 8 families = one warp batch; lane = (family, child).  Siblings/neighbouring pixels sit in
+//    neighbouring lanes (nested order), which keeps opacity gathers and atomics on neighbouring cells.
+//  * Each warp owns a LIFO stack in global memory (depth-first => bounded memory: <= 32 families per
+//    level).  Survivors of a batch are compacted with a ballot/popc prefix and pushed in one step.
+//  * Load balance: root families come from a global seed counter; idle warps raise `hungry` and busy
+//    warps donate the shallow half of their stack (biggest subtrees) through a bounded MPMC ticket queue.
+//  * Deposit: fire-and-forget fp64 REDs into the cell's accumulator record.  The RED path costs
+//    per LANE (one L1 wavefront / L2 sector op each), so lanes of a warp that are in the same cell in the same
+//    iteration - siblings and neighbouring pixels run almost parallel less than a cell apart - are first summed
+//    in registers (match.any on the cell index, shuffles) and one lane issues the REDs for the group.
+//  * Deterministic arithmetic (contract C0-C5): every operation that decides a cell, an axis, a split or a
+//    termination is an explicit IEEE round-to-nearest intrinsic (no FMA contraction), typed from DESIGN.md.
+#pragma once
+#include "arc_internal.cuh"
+#include "arc_healpix.cuh"
+
+#define FLAG_LOG 1          // template flag: per-ray logging (arc_trace_debug)
+#define FLAG_DIGEST 2       // template flag: accumulate the order-independent traversal digest
+
+#ifndef ARC_TRACE_MIN_BLOCKS
+#define ARC_TRACE_MIN_BLOCKS 3     // resident blocks per SM the register budget is held to (<= 85 registers)
+#endif
+#define DEP_RED 1           // every lane: nb fp64 REDs per segment
+#define DEP_AGG 2           // lanes of a warp that sit in the same cell are summed first (match.any + shuffles): one lane REDs
+
+namespace {
+
+__device__ __forceinline__ unsigned long long mix64(unsigned long long x)   // splitmix64 finaliser
+{
+    x ^= x >> 30; x *= 0xbf58476d1ce4e5b9ull;
+    x ^= x >> 27; x *= 0x94d049bb133111ebull;
+    x ^= x >> 31;
+    return x;
+}
+
+__device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned long long *p)
+{
+    return *(const volatile unsigned long long *)p;
+}
+__device__ __forceinline__ long long ld_volatile_s64(const long long *p) { return *(const volatile long long *)p; }
+__device__ __forceinline__ int ld_volatile_s32(const int *p) { return *(const volatile int *)p; }
+
+__device__ __forceinline__ unsigned long long globaltimer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+
+// fire-and-forget fp64 reduction (REDG.E.ADD.F64): written as PTX `red` because ptxas otherwise emits the returning
+// form (ATOMG ... RZ) inside this kernel's divergent loop, which holds a scoreboard until L2 answers
+__device__ __forceinline__ void arc_red_add(double *p, double v)
+{
+    asm volatile("red.relaxed.gpu.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
+}
+
+// opacity gather: the NB opacities of one cell, kept at their storage type until used (fewer registers while
+// the prefetched copy is in flight); one vector load per cell where the layout allows
+template <typename KT, int NB> struct KVec;
+template <int NB> struct KVec<float, NB> {
+    float k[NB];
+    __device__ __forceinline__ void load(const float *base, int cell)
+    {
+        const float *p = base + (long long)cell * NB;
+        if constexpr (NB % 4 == 0) {
+#pragma unroll
+            for (int v = 0; v < NB; v += 4) { const float4 q = __ldg((const float4 *)(p + v)); k[v] = q.x; k[v + 1] = q.y; k[v + 2] = q.z; k[v + 3] = q.w; }
+        } else if constexpr (NB % 2 == 0) {
+#pragma unroll
+            for (int v = 0; v < NB; v += 2) { const float2 q = __ldg((const float2 *)(p + v)); k[v] = q.x; k[v + 1] = q.y; }
+        } else {
+#pragma unroll
+            for (int v = 0; v < NB; ++v) k[v] = __ldg(p + v);
+        }
+    }
+    __device__ __forceinline__ double get(int v) const { return (double)k[v]; }
+};
+template <int NB> struct KVec<double, NB> {
+    double k[NB];
+    __device__ __forceinline__ void load(const double *base, int cell)
+    {
+        const double *p = base + (long long)cell * NB;
+        if constexpr (NB % 2 == 0) {
+#pragma unroll
+            for (int v = 0; v < NB; v += 2) { const double2 q = __ldg((const double2 *)(p + v)); k[v] = q.x; k[v + 1] = q.y; }
+        } else {
+#pragma unroll
+            for (int v = 0; v < NB; ++v) k[v] = __ldg(p + v);
+        }
+    }
+    __device__ __forceinline__ double get(int v) const { return k[v]; }
+};
+
+// E = e^-x and ome = 1 - e^-x for x >= 0, both to ~2e-14 relative - ome also for tiny x, where 1 - E would
+// cancel.  Not a decision: terminations are decided on tau (sums and products only, contract C4).
+// x = -(k ln2 + r) with |r| <= ln2/2;  e^r - 1 = r q(r),  q(r) = sum_{n=0..10} r^n/(n+1)!
+__device__ __forceinline__ void arc_attenuate(double x, double &E, double &ome)
+{
+    const double MAGIC = 6755399441055744.0;                           // 1.5 * 2^52: round to nearest integer
+    const double kt = fma(x, -1.4426950408889634074, MAGIC);
+    const int k = __double2loint(kt);
+    const double kd = kt - MAGIC;
+    double r = fma(kd, -6.93147180369123816490e-01, -x);               // ln2 split in two parts
+    r = fma(kd, -1.90821492927058770002e-10, r);
+    double q = 1.0 / 39916800.0;
+    q = fma(q, r, 1.0 / 3628800.0);
+    q = fma(q, r, 1.0 / 362880.0);
+    q = fma(q, r, 1.0 / 40320.0);
+    q = fma(q, r, 1.0 / 5040.0);
+    q = fma(q, r, 1.0 / 720.0);
+    q = fma(q, r, 1.0 / 120.0);
+    q = fma(q, r, 1.0 / 24.0);
+    q = fma(q, r, 1.0 / 6.0);
+    q = fma(q, r, 0.5);
+    q = fma(q, r, 1.0);
+    const double em1 = r * q;                                          // e^r - 1
+    const double scale = __hiloint2double((max(k, -1022) + 1023) << 20, 0);    // 2^k
+    const double Ek = (x < 708.0) ? fma(em1, scale, scale) : 0.0;
+    E = Ek;
+    ome = (k == 0) ? -em1 : 1.0 - Ek;
+}
+
+// 2^y for y <= 0 on the SFU (ex2.approx.ftz: ~2 ulp, flushes to zero below 2^-126 - exactly what an attenuation
+// factor wants)
+__device__ __forceinline__ float arc_ex2(float y)
+{
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(y));
+    return r;
+}
+
+// ---------------------------------------------------------------------------------------------------
+template <int NB, typename KT, int FLAGS, int DEP>
+__global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_trace_kernel(const TraceArgs a)
+{
+    typedef FamRec<NB> Rec;
+    const int lane = threadIdx.x & 31;
+    const int gwarp = blockIdx.x * ARC_WARPS_PER_BLOCK + (threadIdx.x >> 5);
+    Rec *const stack = reinterpret_cast<Rec *>(a.stacks) + (size_t)gwarp * ARC_STACK_CAP;
+    Rec *const queue = reinterpret_cast<Rec *>(a.queue);
+    SchedState *const sc = a.sched;
+    const KT *const kappa = reinterpret_cast<const KT *>(a.kappa);
+    const int N = a.N;
+    constexpr int NBP = (NB == 1) ? 1 : ((NB + 1) & ~1);      // accumulator record stride (arc_nbp)
+    unsigned long long nred = 0;                              // deposit records this lane sent to L2
+
+    __shared__ unsigned long long s_splits[ARC_MAX_LEVEL], s_rays[ARC_MAX_LEVEL], s_ends[3];
+    __shared__ double s_esc[ARC_MAX_BINS];
+    __shared__ double s_geo[6][ARC_TRACE_THREADS];            // per thread: source position g[3], direction d[3]
+    if (threadIdx.x < ARC_MAX_LEVEL) { s_splits[threadIdx.x] = 0; s_rays[threadIdx.x] = 0; }
+    if (threadIdx.x < 3) s_ends[threadIdx.x] = 0;
+    if (threadIdx.x < ARC_MAX_BINS) s_esc[threadIdx.x] = 0.0;
+    __syncthreads();
+
+    // own stack = ring of ARC_STACK_CAP records holding families [bot, top) (monotonic counters, warp-uniform)
+    unsigned bot = 0, top = 0;
+#define STK(i) stack[(i) & (ARC_STACK_CAP - 1)]
+    long long delta = 0;                  // families created - consumed since the last flush (warp-uniform)
+    unsigned long long nseg = 0, digest = 0;
+    bool registered_hungry = false;
+    bool quit = false;
+
+    while (!quit) {
+        // ------------------------------------------------------------------ acquire work
+        if (top == bot) {
+            if (delta != 0) { if (lane == 0) atomicAdd((unsigned long long *)&sc->in_flight, (unsigned long long)delta); delta = 0; }
+            unsigned long long t_idle0 = 0; long long last_seen = 0; unsigned backoff = 64;
+            for (;;) {
+                // (1) donated families: claim up to `want` published entries from the counting semaphore
+                // q_count, then take that many consecutive tickets.  No retry loops: every atomic succeeds.
+                int n = 0; unsigned long long ticket = 0;
+                if (lane == 0) {
+                    const long long avail = ld_volatile_s64(&sc->q_count);
+                    if (avail > 0) {
+                        const int hungry_now = max(ld_volatile_s32(&sc->hungry), 1);
+                        const long long want = max(1ll, min((long long)ARC_BATCH_FAM, avail / hungry_now));
+                        const long long before = (long long)atomicAdd((unsigned long long *)&sc->q_count, (unsigned long long)(-want));
+                        const long long got = max(0ll, min(before, want));
+                        if (got < want) atomicAdd((unsigned long long *)&sc->q_count, (unsigned long long)(want - got));
+                        if (got > 0) { ticket = atomicAdd(&sc->q_head, (unsigned long long)got); n = (int)got; }
+                    }
+                }
+                n = __shfl_sync(0xffffffffu, n, 0);
+                ticket = __shfl_sync(0xffffffffu, ticket, 0);
+                if (n > 0) {
+                    if (lane < n) {
+                        const unsigned long long tk = ticket + lane;
+                        const unsigned slot = (unsigned)(tk % ARC_QUEUE_CAP);
+                        while (ld_volatile_u64(&a.qseq[slot]) != tk + 1) __nanosleep(32);
+                        __threadfence();
+                        const int4 *src = reinterpret_cast<const int4 *>(&queue[slot]);
+                        int4 *dst = reinterpret_cast<int4 *>(&STK(top + lane));
+#pragma unroll
+                        for (int w = 0; w < (int)(sizeof(Rec) / 16); ++w) dst[w] = __ldcg(src + w);
+                        __threadfence();
+                        *(volatile unsigned long long *)&a.qseq[slot] = tk + ARC_QUEUE_CAP;   // slot free for the next lap
+                    }
+                    top += n;
+                    break;
+                }
+                // (2) root families (a3: r = 0, tau = 0)
+                unsigned long long s0 = 0;
+                if (lane == 0 && ld_volatile_u64(&sc->seed_next) < a.seed_total) {
+                    s0 = atomicAdd(&sc->seed_next, (unsigned long long)a.seed_chunk);
+                    if (s0 < a.seed_total) n = (int)min((unsigned long long)a.seed_chunk, a.seed_total - s0);
+                }
+                n = __shfl_sync(0xffffffffu, n, 0);
+                s0 = __shfl_sync(0xffffffffu, s0, 0);
+                if (n > 0) {
+                    if (lane < n) {
+                        Rec r;
+                        const unsigned long long s = s0 + lane;
+                        r.src = (uint32_t)(s / a.fam_per_src); r.fam = (uint32_t)(s % a.fam_per_src);
+                        r.level = (uint32_t)a.l0; r.pad = 0;
+#pragma unroll
+                        for (int v = 0; v < NB; ++v) r.tau[v] = 0.0;
+                        STK(top + lane) = r;
+                    }
+                    top += n;
+                    break;
+                }
+                // (3) nothing to do: wait for donations or for the end
+                if (!registered_hungry) { if (lane == 0) atomicAdd(&sc->hungry, 1); registered_hungry = true; }
+                int stop = 0;
+                if (lane == 0) {
+                    const long long inflight = ld_volatile_s64(&sc->in_flight);
+                    if (inflight == 0 || ld_volatile_s32(&sc->error) != 0) stop = 1;
+                    else {
+                        const unsigned long long now = globaltimer_ns();
+                        if (t_idle0 == 0 || inflight != last_seen) { t_idle0 = now; last_seen = inflight; }
+                        else if (now - t_idle0 > 20000000000ull) { atomicCAS(&sc->error, 0, ARC_DEV_WATCHDOG); stop = 1; }
+                    }
+                }
+                stop = __shfl_sync(0xffffffffu, stop, 0);
+                if (stop) { quit = true; break; }
+                __nanosleep(backoff);
+                if (backoff < 2048) backoff *= 2;
+            }
+            if (registered_hungry && !quit) { if (lane == 0) atomicSub(&sc->hungry, 1); registered_hungry = false; }
+            if (quit) break;
+            __syncwarp();
+        }
+
+        // ------------------------------------------------------------------ pop a batch: lane = (family, child)
+        const int nfam = (int)min((unsigned)ARC_BATCH_FAM, top - bot);
+        top -= nfam;
+        const int myfam = lane >> 2;
+        bool active = myfam < nfam;
+        uint32_t src = 0, pix = 0; int level = 0;
+        double tau[NB], P[NB];
+        const double INF = __longlong_as_double(0x7ff0000000000000ll);
+        double tx = INF, ty = INF, tz = INF, r = 0, r_end = 0;
+        unsigned ijk = 0;                      // cell coordinates, 10 bits each (N <= 1024)
+        int cell = 0;                          // N <= 1024: N^3 <= 2^30
+        int end = -1;
+        unsigned long long h = 0; unsigned int seq = 0;
+        if (active) {
+            const Rec *rp = &STK(top + myfam);
+            src = rp->src; level = (int)rp->level; pix = 4u * rp->fam + (uint32_t)(lane & 3);
+#pragma unroll
+            for (int v = 0; v < NB; ++v) tau[v] = rp->tau[v];
+            double dirx, diry, dirz;
+            arc_pix2vec_dev(level, pix, dirx, diry, dirz);
+            const double gx = __ldg(a.src_g + 3 * src), gy = __ldg(a.src_g + 3 * src + 1), gz = __ldg(a.src_g + 3 * src + 2);
+            // the ray's constants live in shared memory (read back by this thread only: no barrier needed); the
+            // loop fetches just the crossed axis' pair, which keeps 12 registers free for a third resident block
+            s_geo[0][threadIdx.x] = gx; s_geo[1][threadIdx.x] = gy; s_geo[2][threadIdx.x] = gz;
+            s_geo[3][threadIdx.x] = dirx; s_geo[4][threadIdx.x] = diry; s_geo[5][threadIdx.x] = dirz;
+            const double npix = (double)(12ull << (2 * level));
+#pragma unroll
+            for (int v = 0; v < NB; ++v) P[v] = (__ldg(a.src_S + (size_t)src * NB + v) / npix) * exp(-tau[v]);
+            // split radii: exact power-of-two scalings of csplit (O2)
+            r = (level == a.l0) ? 0.0 : scalbn(a.csplit, level - 1);
+            r_end = (level >= a.Lmax) ? INF : scalbn(a.csplit, level);
+            // a5: starting cell (O3 step 2)
+            const double x0 = arc_add(gx, arc_mul(r, dirx)), y0 = arc_add(gy, arc_mul(r, diry)), z0 = arc_add(gz, arc_mul(r, dirz));
+            double fx = floor(x0), fy = floor(y0), fz = floor(z0);
+            if (x0 == fx && dirx < 0.0) fx -= 1.0;
+            if (y0 == fy && diry < 0.0) fy -= 1.0;
+            if (z0 == fz && dirz < 0.0) fz -= 1.0;
+            const double dN = (double)N;
+            const bool inside = fx >= 0.0 && fx < dN && fy >= 0.0 && fy < dN && fz >= 0.0 && fz < dN;
+            if (FLAGS & FLAG_DIGEST) h = mix64(((unsigned long long)src << 40) | ((unsigned long long)level << 32) | pix);
+            atomicAdd(&s_rays[level], 1ull);
+            if (!inside) {
+#pragma unroll
+                for (int v = 0; v < NB; ++v) atomicAdd(&s_esc[v], P[v]);
+                end = ARC_END_ESCAPED; active = false;
+            } else {
+                const int ix = (int)fx, iy = (int)fy, iz = (int)fz;
+                ijk = (unsigned)ix | ((unsigned)iy << 10) | ((unsigned)iz << 20);
+                cell = (iz * N + iy) * N + ix;
+                if (dirx != 0.0) tx = __ddiv_rn(arc_sub((double)(ix + (dirx > 0.0)), gx), dirx);
+                if (diry != 0.0) ty = __ddiv_rn(arc_sub((double)(iy + (diry > 0.0)), gy), diry);
+                if (dirz != 0.0) tz = __ddiv_rn(arc_sub((double)(iz + (dirz > 0.0)), gz), dirz);
+            }
+        }
+
+        // ------------------------------------------------------------------ a6/a7: the segment loop
+        // One warp iteration = one (ray, cell) segment per active lane.  Everything that is per axis is selected once
+        // (the crossed axis), the advance costs one IEEE division, the next cell's opacities are requested before this
+        // segment's attenuation arithmetic, and the state advance is unconditional (a lane that just ended is inactive).
+        const unsigned int max_seg = 3u * (unsigned)N + 8u;
+        unsigned int nray_seg = 0, nseg_b = 0, nred_b = 0;
+        KVec<KT, NB> kcur;
+        kcur.load(kappa, cell);                 // (cell 0 for lanes without a ray: harmless)
+        for (;;) {
+          if (!__any_sync(0xffffffffu, active)) break;
+          double av[NB];
+          int dcell = -1 - lane;                 // deposit key; lanes without a segment keep a unique negative one
+          if (active) {
+            // a6: first face crossed; ties go to x, then y (reading G9)
+            int ax = 0; double tmin = tx;
+            if (ty < tmin) { tmin = ty; ax = 1; }
+            if (tz < tmin) { tmin = tz; ax = 2; }
+            const bool split = (r_end <= tmin);
+            const double r_out = split ? r_end : tmin;
+            const double ds = arc_sub(r_out, r);
+            const double dl = arc_mul(ds > 0.0 ? ds : 0.0, a.dx);
+            const double g_ax = s_geo[ax][threadIdx.x], d_ax = s_geo[3 + ax][threadIdx.x];
+            const int pos = (__double2hiint(d_ax) >= 0) ? 1 : 0;          // d_ax > 0 (it is never zero on the crossed axis)
+            const int st = 2 * pos - 1;
+            const int sh = 10 * ax;
+            const int inext = (int)((ijk >> sh) & 1023u) + st;
+            const bool out = (unsigned)inext >= (unsigned)N;
+            const int stride = ax == 0 ? 1 : (ax == 1 ? N : N * N);
+            const int cell_next = cell + st * stride;
+            const bool go = !(split || out);
+            KVec<KT, NB> knext;
+            knext.load(kappa, go ? cell_next : cell);                       // always a valid cell: no divergence here
+            const double t_new = __ddiv_rn(arc_sub((double)(inext + pos), g_ax), d_ax);
+            // a7: optical depth (fp64, decides: contract C4) and the deposit of Eq. 1
+            bool depleted = true;
+            if constexpr (sizeof(KT) == 4) {
+                // fp32-field mode (tolerance 1e-3): the attenuation FACTOR is evaluated in fp32, everything that carries
+                // or decides stays fp64.  Thin segment: absorbed = P ome, kept = P - absorbed; thick: kept = P E,
+                // absorbed = P - kept - either way absorbed + kept = P exactly, and the small one is the accurate one.
+                const float dlf = (float)dl;
+#pragma unroll
+                for (int v = 0; v < NB; ++v) {
+                    const double dtau = arc_mul(kcur.get(v), dl);
+                    tau[v] = arc_add(tau[v], dtau);
+                    depleted = depleted && (tau[v] >= a.tau_term);       // min_nu tau_nu >= tau_term
+                    const float x = kcur.k[v] * dlf;
+                    float p = 1.0f / 720.0f;                             // ome = x (1 - x/2 + x^2/6 - ... + x^5/720), x < 1/8
+                    p = fmaf(p, x, -1.0f / 120.0f);
+                    p = fmaf(p, x, 1.0f / 24.0f);
+                    p = fmaf(p, x, -1.0f / 6.0f);
+                    p = fmaf(p, x, 0.5f);
+                    p = fmaf(-p, x, 1.0f);
+                    const bool thin = x < 0.125f;
+                    const float f = thin ? p * x : arc_ex2(-1.4426950408889634f * x);
+                    const double q = P[v] * (double)f;
+                    const double rest = P[v] - q;
+                    av[v] = thin ? q : rest;
+                    P[v] = thin ? rest : q;
+                }
+            } else {
+#pragma unroll
+                for (int v = 0; v < NB; ++v) {
+                    const double dtau = arc_mul(kcur.get(v), dl);
+                    tau[v] = arc_add(tau[v], dtau);
+                    depleted = depleted && (tau[v] >= a.tau_term);
+                    double E, ome;
+                    arc_attenuate(dtau, E, ome);                // e^-dtau and 1 - e^-dtau
+                    av[v] = P[v] * ome;                         // absorbed = P (1 - e^-dtau)
+                    P[v] = P[v] * E;                            // photon conserving: the ray keeps P e^-dtau
+                }
+            }
+            if (depleted) {
+#pragma unroll
+                for (int v = 0; v < NB; ++v) av[v] += P[v];     // reading G7: the remainder stays in this cell
+            }
+            dcell = cell;
+            ++nseg_b; ++nray_seg;
+            if (FLAGS & FLAG_DIGEST) h = mix64(h ^ (unsigned long long)cell);
+            if (FLAGS & FLAG_LOG) {
+                const unsigned long long e = atomicAdd(&sc->log_n, 1ull);
+                if (e < a.log_cap) {
+                    a.log_key[e] = ((unsigned long long)src << 40) | ((unsigned long long)level << 32) | pix;
+                    a.log_seq[e] = seq; a.log_cell[e] = cell;
+                }
+                ++seq;
+            }
+            if (depleted || !go || nray_seg > max_seg) {
+                active = false;
+                if (depleted) end = ARC_END_DEPLETED;
+                else if (split) end = ARC_END_SPLIT;
+                else {
+                    if (!out) atomicCAS(&sc->error, 0, ARC_DEV_RAY_RUNAWAY);
+#pragma unroll
+                    for (int v = 0; v < NB; ++v) atomicAdd(&s_esc[v], P[v]);
+                    end = ARC_END_ESCAPED;
+                }
+            }
+            // unconditional advance
+            r = r_out; cell = cell_next; kcur = knext;
+            ijk += (unsigned)st << sh;
+            tx = (ax == 0) ? t_new : tx;
+            ty = (ax == 1) ? t_new : ty;
+            tz = (ax == 2) ? t_new : tz;
+          }
+          // a7: deposit - the whole warp, converged
+          if constexpr (DEP == DEP_AGG) {
+              // segmented sum over the lanes that share a cell, by pointer jumping along each group's lane list:
+              // after ceil(log2(group size)) rounds the first lane of a group holds the group's sum
+              const unsigned peers = __match_any_sync(0xffffffffu, dcell);
+              const int leader = __ffs(peers) - 1;
+              int nxt = __ffs(peers & ~((2u << lane) - 1u)) - 1;          // next lane of my group, -1 at the tail
+              while (__any_sync(0xffffffffu, nxt >= 0)) {
+                  const int from = nxt >= 0 ? nxt : lane;
+#pragma unroll
+                  for (int v = 0; v < NB; ++v) {
+                      const double o = __shfl_sync(0xffffffffu, av[v], from);
+                      if (nxt >= 0) av[v] += o;
+                  }
+                  nxt = __shfl_sync(0xffffffffu, nxt, from);              // (a tail lane reads its own -1)
+              }
+              if (lane == leader && dcell >= 0) {
+                  double *Ac = a.A + (long long)dcell * NBP;
+#pragma unroll
+                  for (int v = 0; v < NB; ++v) arc_red_add(Ac + v, av[v]);
+                  ++nred_b;
+              }
+          } else {
+              if (dcell >= 0) {
+                  double *Ac = a.A + (long long)dcell * NBP;
+#pragma unroll
+                  for (int v = 0; v < NB; ++v) arc_red_add(Ac + v, av[v]);   // a7: REDG.E.ADD.F64 ("atomically")
+                  ++nred_b;
+              }
+          }
+        }
+        nseg += nseg_b; nred += nred_b;
+        __syncwarp();
+
+        // ------------------------------------------------------------------ a8/a9: bookkeeping, push children
+        if (end >= 0) {
+            atomicAdd(&s_ends[end], 1ull);
+            if (FLAGS & FLAG_DIGEST) { h = mix64(h ^ (0xE0ull + (unsigned long long)end)); digest += h; }
+            if (FLAGS & FLAG_LOG) {
+                const unsigned long long e = atomicAdd(&sc->log_n, 1ull);
+                if (e < a.log_cap) {
+                    a.log_key[e] = ((unsigned long long)src << 40) | ((unsigned long long)level << 32) | pix;
+                    a.log_seq[e] = seq; a.log_cell[e] = -1 - end;
+                }
+            }
+        }
+        const bool do_split = (end == ARC_END_SPLIT);
+        if (do_split) atomicAdd(&s_splits[level], 1ull);
+        const unsigned ballot = __ballot_sync(0xffffffffu, do_split);
+        const int npush = __popc(ballot);
+        if (top - bot + npush > ARC_STACK_CAP) {
+            if (lane == 0) atomicCAS(&sc->error, 0, ARC_DEV_STACK_OVERFLOW);
+            quit = true;
+        } else {
+            if (do_split) {
+                const int rank = __popc(ballot & ((1u << lane) - 1u));
+                Rec rec;
+                rec.src = src; rec.fam = pix; rec.level = (uint32_t)(level + 1); rec.pad = 0;
+#pragma unroll
+                for (int v = 0; v < NB; ++v) rec.tau[v] = tau[v];
+                STK(top + rank) = rec;
+            }
+            top += npush;
+            delta += (long long)npush - nfam;
+        }
+        __syncwarp();
+
+        // ------------------------------------------------------------------ donate the shallow half if someone is idle
+        int hungry = 0, err = 0;
+        if (lane == 0) { hungry = ld_volatile_s32(&sc->hungry); err = ld_volatile_s32(&sc->error); }
+        hungry = __shfl_sync(0xffffffffu, hungry, 0);
+        err = __shfl_sync(0xffffffffu, err, 0);
+        if (err) quit = true;
+        if (!quit && hungry > 0 && top - bot >= 2) {
+            int nd = (int)min((top - bot) / 2, 32u);
+            unsigned long long ticket = 0;
+            if (lane == 0) {
+                // donate only while the pool is short of what the idle warps can take; the level test is
+                // approximate (plain loads), the ring is sized so that every warp overshooting at once still fits
+                const unsigned long long t = ld_volatile_u64(&sc->q_tail), hq = ld_volatile_u64(&sc->q_head);
+                const unsigned long long level_now = t > hq ? t - hq : 0ull;
+                if (level_now >= (unsigned long long)min(hungry * 4, ARC_QUEUE_LOW)) nd = 0;
+                else {
+                    // flush first: donated families must be covered by the global counter before they are visible
+                    if (delta != 0) atomicAdd((unsigned long long *)&sc->in_flight, (unsigned long long)delta);
+                    ticket = atomicAdd(&sc->q_tail, (unsigned long long)nd);
+                    atomicMax(&sc->q_high, ticket + nd - hq);
+                }
+            }
+            nd = __shfl_sync(0xffffffffu, nd, 0);
+            ticket = __shfl_sync(0xffffffffu, ticket, 0);
+            if (nd > 0) {
+                delta = 0;
+                if (lane < nd) {
+                    const unsigned long long tk = ticket + lane;
+                    const unsigned slot = (unsigned)(tk % ARC_QUEUE_CAP);
+                    while (ld_volatile_u64(&a.qseq[slot]) != tk) __nanosleep(32);    // previous lap's reader finished
+                    const int4 *s4 = reinterpret_cast<const int4 *>(&STK(bot + lane));
+                    int4 *d4 = reinterpret_cast<int4 *>(&queue[slot]);
+#pragma unroll
+                    for (int w = 0; w < (int)(sizeof(Rec) / 16); ++w) __stcg(d4 + w, s4[w]);
+                    __threadfence();
+                    *(volatile unsigned long long *)&a.qseq[slot] = tk + 1;            // publish
+                }
+                __syncwarp();
+                if (lane == 0) atomicAdd((unsigned long long *)&sc->q_count, (unsigned long long)nd);
+            }
+            bot += nd;
+            __syncwarp();
+        }
+    }
+
+    // ---------------------------------------------------------------------- flush statistics
+    if (registered_hungry && lane == 0) atomicSub(&sc->hungry, 1);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        nseg += __shfl_xor_sync(0xffffffffu, nseg, o);
+        nred += __shfl_xor_sync(0xffffffffu, nred, o);
+        digest += __shfl_xor_sync(0xffffffffu, digest, o);
+    }
+    if (lane == 0) {
+        atomicAdd(&a.stats->segments, nseg);
+        atomicAdd(&a.stats->deposit_records, nred);
+        if (FLAGS & FLAG_DIGEST) atomicAdd(&a.stats->digest, digest);
+    }
+    __syncthreads();
+    if (threadIdx.x < ARC_MAX_LEVEL) {
+        if (s_splits[threadIdx.x]) atomicAdd(&a.stats->splits[threadIdx.x], s_splits[threadIdx.x]);
+        if (s_rays[threadIdx.x]) { atomicAdd(&a.stats->rays_level[threadIdx.x], s_rays[threadIdx.x]); atomicAdd(&a.stats->rays, s_rays[threadIdx.x]); }
+    }
+    if (threadIdx.x < 3 && s_ends[threadIdx.x]) atomicAdd(&a.stats->ends[threadIdx.x], s_ends[threadIdx.x]);
+    if (threadIdx.x < NB && s_esc[threadIdx.x] != 0.0) atomicAdd(&a.stats->escaped[threadIdx.x], s_esc[threadIdx.x]);
+}
+
+template <int NB, typename KT, int DEP>
+cudaError_t launch_dep(const TraceArgs &a, bool log, int grid, cudaStream_t s)
+{
+    if (log) arc_trace_kernel<NB, KT, FLAG_LOG | FLAG_DIGEST, DEP><<<grid, ARC_TRACE_THREADS, 0, s>>>(a);
+    else if (a.flags & FLAG_DIGEST) arc_trace_kernel<NB, KT, FLAG_DIGEST, DEP><<<grid, ARC_TRACE_THREADS, 0, s>>>(a);
+    else arc_trace_kernel<NB, KT, 0, DEP><<<grid, ARC_TRACE_THREADS, 0, s>>>(a);
+    return cudaGetLastError();
+}
+
+template <int NB, typename KT>
+cudaError_t launch_nb(const TraceArgs &a, bool log, int dep, int grid, cudaStream_t s)
+{
+    switch (dep) {
+        case DEP_AGG: return launch_dep<NB, KT, DEP_AGG>(a, log, grid, s);
+        default: return launch_dep<NB, KT, DEP_RED>(a, log, grid, s);
+    }
+}
+
+template <int NB, typename KT, int DEP>
+int occ_dep(int flags)
+{
+    int nblk = 0;
+    cudaError_t e;
+    if (flags & FLAG_LOG) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, arc_trace_kernel<NB, KT, FLAG_LOG | FLAG_DIGEST, DEP>, ARC_TRACE_THREADS, 0);
+    else if (flags & FLAG_DIGEST) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, arc_trace_kernel<NB, KT, FLAG_DIGEST, DEP>, ARC_TRACE_THREADS, 0);
+    else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, arc_trace_kernel<NB, KT, 0, DEP>, ARC_TRACE_THREADS, 0);
+    if (e != cudaSuccess) { cudaGetLastError(); return 1; }
+    return nblk < 1 ? 1 : nblk;
+}
+
+template <int NB, typename KT>
+int occ_nb(int dep, int flags)
+{
+    return dep == DEP_AGG ? occ_dep<NB, KT, DEP_AGG>(flags) : occ_dep<NB, KT, DEP_RED>(flags);
+}
+
+}  // namespace
+
+// One translation unit per (opacity dtype, half of the bin range): ARC_INST_KT, ARC_INST_NB0 (1 or 5), ARC_INST_TAG
+#define ARC_CAT2(a, b) a##b
+#define ARC_CAT(a, b) ARC_CAT2(a, b)
+
+cudaError_t ARC_CAT(arc_trace_launch_, ARC_INST_TAG)(const TraceArgs &a, bool log, int dep, int grid, cudaStream_t s)
+{
+    switch (a.nb - ARC_INST_NB0) {
+        case 0: return launch_nb<ARC_INST_NB0 + 0, ARC_INST_KT>(a, log, dep, grid, s);
+        case 1: return launch_nb<ARC_INST_NB0 + 1, ARC_INST_KT>(a, log, dep, grid, s);
+        case 2: return launch_nb<ARC_INST_NB0 + 2, ARC_INST_KT>(a, log, dep, grid, s);
+        case 3: return launch_nb<ARC_INST_NB0 + 3, ARC_INST_KT>(a, log, dep, grid, s);
+    }
+    return cudaErrorInvalidValue;
+}
+
+int ARC_CAT(arc_trace_occ_, ARC_INST_TAG)(int nb, int dep, int flags)
+{
+    switch (nb - ARC_INST_NB0) {
+        case 0: return occ_nb<ARC_INST_NB0 + 0, ARC_INST_KT>(dep, flags);
+        case 1: return occ_nb<ARC_INST_NB0 + 1, ARC_INST_KT>(dep, flags);
+        case 2: return occ_nb<ARC_INST_NB0 + 2, ARC_INST_KT>(dep, flags);
+        case 3: return occ_nb<ARC_INST_NB0 + 3, ARC_INST_KT>(dep, flags);
+    }
+    return 1;
+}

@@ -62,4 +62,4 @@ def run_gpu_trace(w, fields=None, **override):
 
 
 def oracle_override(override):
-    return {k: v for k, v in override.items() if k not in ("digest", "async", "trace_blocks")}
+    return {k: v for k, v in override.items() if k not in ("digest", "async", "trace_blocks", "deposit")}
