@@ -150,6 +150,25 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# ------------------------------------------------------------------------------------------------ ranks
+def reduce_over_ranks(times_ms, counts, device, world):
+    """Replicas only: every rank runs the whole workload on its own GPU and nothing of the data path
+    crosses ranks.  The job's time is the MAX over ranks of each device-timed interval, its work the SUM over ranks
+    of the units processed.  -> (list of max times, list of summed counts)"""
+    import torch
+    t = torch.tensor([float(x) for x in times_ms], dtype=torch.float64, device=device)
+    s = torch.tensor([float(x) for x in counts], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(s, op=dist.ReduceOp.SUM)
+    return t.tolist(), s.tolist()
+
+
+def job_throughput(units_all_ranks, ms_max_over_ranks):
+    return units_all_ranks / (ms_max_over_ranks * 1e-3) if ms_max_over_ranks > 0 else 0.0
+
+
 # ------------------------------------------------------------------------------------------------ CUDA arm
 def run_cuda(args):
     import torch
@@ -247,25 +266,19 @@ def run_cuda(args):
 
     # ---- reduce over ranks (replicas: every rank ran the same workload on its own GPU)
     tot_seg = float(sum(seg_steps))
-    t = torch.tensor([dev_ms, e2e_ms], dtype=torch.float64, device="cuda")
-    s = torch.tensor([tot_seg, float(e2e_seg)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(s, op=dist.ReduceOp.SUM)
-    dev_ms_max, e2e_ms_max = float(t[0]), float(t[1])
-    seg_all, e2e_seg_all = float(s[0]), float(s[1])
+    (dev_ms_max, e2e_ms_max), (seg_all, e2e_seg_all) = reduce_over_ranks([dev_ms, e2e_ms], [tot_seg, float(e2e_seg)], "cuda", world)
 
     if rank == 0:
         kms = float(sum(kern_ms))
         achieved = bytes_seg * tot_seg / (kms * 1e-3) / 1e9 if kms > 0 else 0.0
         line = {
-            "metric": METRIC, "value": seg_all / (dev_ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "metric": METRIC, "value": job_throughput(seg_all, dev_ms_max), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, paper_1807_07094_b200/workloads.py)",
             "config": dict(describe(w), parallelism="replicas" if world > 1 else "single-gpu",
                            l2_policy="inputs larger than L2" if (nc * nb * (bytes_seg // nb)) > 126e6 else "working set fits L2 (small config)",
                            trace_grid_blocks=trace_grid, deposit=args.deposit),
-            "e2e": {"value": e2e_seg_all / (e2e_ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "e2e": {"value": job_throughput(e2e_seg_all, e2e_ms_max), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": 5 * args.steps,
             "clocks": clocks,
             "roofline": {"bound": "hbm", "kernel": "arc_trace_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",

@@ -143,6 +143,11 @@ def arc_version() -> str:
     return lib().arc_version().decode()
 
 
+def arc_last_error(ctx=None) -> str:
+    """Text of the last failure of `ctx` (None: of the last failed arc_create_grid on this thread)."""
+    return (lib().arc_last_error(ctx) or b"").decode()
+
+
 def arc_create_grid(N: int, box_cm: float, dtype: int):
     ctx = C.c_void_p()
     rc = lib().arc_create_grid(C.byref(ctx), int(N), float(box_cm), int(dtype))

@@ -17,7 +17,10 @@
 enum { ARC_DEV_OK = 0, ARC_DEV_STACK_OVERFLOW = 1, ARC_DEV_LOG_OVERFLOW = 2, ARC_DEV_WATCHDOG = 3, ARC_DEV_RAY_RUNAWAY = 4 };
 
 // A "family" = the 4 children 4*fam+j (j = 0..3) of one split (or 4 consecutive root pixels), all at
-// `level`, starting at the parent's split radius with the parent's optical depths.
+// `level`, starting at the parent's split radius with the parent's optical depths.  P is the
+// photon rate each child still carries, S_nu e^-tau_nu / npix = a quarter of what the parent had left: handing the
+// carried value down (instead of re-deriving it from tau) makes emitted = absorbed + escaped hold to rounding
+// whatever precision the attenuation factor was evaluated in.
 template <int NB>
 struct __align__(16) FamRec {
     uint32_t src;
@@ -25,6 +28,7 @@ struct __align__(16) FamRec {
     uint32_t level;
     uint32_t pad;
     double tau[NB];
+    double P[NB];
 };
 
 struct SchedState {

@@ -18,7 +18,7 @@
 
 static int fail(arc_ctx *c, int code, const std::string &msg) { c->err = msg; return code; }
 
-static size_t famrec_bytes(int nb) { return (size_t)((16 + 8 * nb + 15) / 16) * 16; }
+static size_t famrec_bytes(int nb) { return (size_t)(16 + 16 * nb); }      // sizeof(FamRec<nb>)
 
 // check the device-side error word after a synchronised trace
 static int device_error(arc_ctx *c)

@@ -224,8 +224,9 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                         const unsigned long long s = s0 + lane;
                         r.src = (uint32_t)(s / a.fam_per_src); r.fam = (uint32_t)(s % a.fam_per_src);
                         r.level = (uint32_t)a.l0; r.pad = 0;
+                        const double npix0 = (double)(12ull << (2 * a.l0));
 #pragma unroll
-                        for (int v = 0; v < NB; ++v) r.tau[v] = 0.0;
+                        for (int v = 0; v < NB; ++v) { r.tau[v] = 0.0; r.P[v] = __ldg(a.src_S + (size_t)r.src * NB + v) / npix0; }
                         STK(top + lane) = r;
                     }
                     top += n;
@@ -270,7 +271,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
             const Rec *rp = &STK(top + myfam);
             src = rp->src; level = (int)rp->level; pix = 4u * rp->fam + (uint32_t)(lane & 3);
 #pragma unroll
-            for (int v = 0; v < NB; ++v) tau[v] = rp->tau[v];
+            for (int v = 0; v < NB; ++v) { tau[v] = rp->tau[v]; P[v] = rp->P[v]; }
             double dirx, diry, dirz;
             arc_pix2vec_dev(level, pix, dirx, diry, dirz);
             const double gx = __ldg(a.src_g + 3 * src), gy = __ldg(a.src_g + 3 * src + 1), gz = __ldg(a.src_g + 3 * src + 2);
@@ -278,9 +279,6 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
             // loop fetches just the crossed axis' pair, which keeps 12 registers free for a third resident block
             s_geo[0][threadIdx.x] = gx; s_geo[1][threadIdx.x] = gy; s_geo[2][threadIdx.x] = gz;
             s_geo[3][threadIdx.x] = dirx; s_geo[4][threadIdx.x] = diry; s_geo[5][threadIdx.x] = dirz;
-            const double npix = (double)(12ull << (2 * level));
-#pragma unroll
-            for (int v = 0; v < NB; ++v) P[v] = (__ldg(a.src_S + (size_t)src * NB + v) / npix) * exp(-tau[v]);
             // split radii: exact power-of-two scalings of csplit (O2)
             r = (level == a.l0) ? 0.0 : scalbn(a.csplit, level - 1);
             r_end = (level >= a.Lmax) ? INF : scalbn(a.csplit, level);
@@ -471,7 +469,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                 Rec rec;
                 rec.src = src; rec.fam = pix; rec.level = (uint32_t)(level + 1); rec.pad = 0;
 #pragma unroll
-                for (int v = 0; v < NB; ++v) rec.tau[v] = tau[v];
+                for (int v = 0; v < NB; ++v) { rec.tau[v] = tau[v]; rec.P[v] = 0.25 * P[v]; }     // each child: a quarter
                 STK(top + rank) = rec;
             }
             top += npush;
