@@ -32,6 +32,9 @@
 #ifndef ARC_TRACE_MIN_BLOCKS
 #define ARC_TRACE_MIN_BLOCKS 3     // resident blocks per SM the register budget is held to (<= 85 registers)
 #endif
+#ifndef ARC_AGG_STEPS
+#define ARC_AGG_STEPS 3            // warp-aggregated deposit: runs of up to 2^ARC_AGG_STEPS neighbouring lanes (0: match.any groups)
+#endif
 #define DEP_RED 1           // every lane: nb fp64 REDs per segment
 #define DEP_AGG 2           // lanes of a warp that sit in the same cell are summed first (match.any + shuffles): one lane REDs
 
@@ -132,6 +135,48 @@ __device__ __forceinline__ void arc_attenuate(double x, double &E, double &ome)
     ome = (k == 0) ? -em1 : 1.0 - Ek;
 }
 
+// a / b rounded to nearest, bit-identical to IEEE division, given y = RN(1 / b) (one true division per ray and axis):
+// q0 = RN(a y) is within 1.5 ulp of a/b; one residual correction q1 = RN(q0 + (a - b q0) y) makes it faithful, and
+// for a faithful q1 and a correctly rounded y the second correction returns RN(a / b) (Markstein 1990, the closing
+// step of the IA-64 division sequences).  The residuals are exact (FMA).  No overflow / underflow here: |a| <= 2N,
+// 2^-40 < |b| <= 1.  Five FP64 instructions instead of the ~17 of the generic division.
+__device__ __forceinline__ double arc_div_by_recip(double a, double b, double y)
+{
+    const double q0 = __dmul_rn(a, y);
+    const double q1 = __fma_rn(__fma_rn(-b, q0, a), y, q0);
+    return __fma_rn(__fma_rn(-b, q1, a), y, q1);
+}
+
+// x += o under a predicate: one predicated DADD (the compiler's own choice is DADD + two selects)
+__device__ __forceinline__ void arc_add_if(double &x, double o, int take)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %2, 0;\n\t@p add.rn.f64 %0, %0, %1;\n\t}" : "+d"(x) : "d"(o), "r"(take));
+}
+
+// two fp32 lanes per instruction (FMUL2 / FFMA2 on sm_100)
+__device__ __forceinline__ unsigned long long arc_pack2(float lo, float hi)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void arc_unpack2(unsigned long long r, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(r));
+}
+__device__ __forceinline__ unsigned long long arc_mul2(unsigned long long a, unsigned long long b)
+{
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ unsigned long long arc_fma2(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+
 // 2^y for y <= 0 on the SFU (ex2.approx.ftz: ~2 ulp, flushes to zero below 2^-126 - exactly what an attenuation
 // factor wants)
 __device__ __forceinline__ float arc_ex2(float y)
@@ -154,11 +199,12 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
     const KT *const kappa = reinterpret_cast<const KT *>(a.kappa);
     const int N = a.N;
     constexpr int NBP = (NB == 1) ? 1 : ((NB + 1) & ~1);      // accumulator record stride (arc_nbp)
+    constexpr int NBE = (NB + 1) & ~1;                        // bins rounded up to whole fp32 pairs
     unsigned long long nred = 0;                              // deposit records this lane sent to L2
 
     __shared__ unsigned long long s_splits[ARC_MAX_LEVEL], s_rays[ARC_MAX_LEVEL], s_ends[3];
     __shared__ double s_esc[ARC_MAX_BINS];
-    __shared__ double s_geo[6][ARC_TRACE_THREADS];            // per thread: source position g[3], direction d[3]
+    __shared__ double s_geo[9][ARC_TRACE_THREADS];            // per thread: source position g[3], direction d[3], RN(1/d)[3]
     if (threadIdx.x < ARC_MAX_LEVEL) { s_splits[threadIdx.x] = 0; s_rays[threadIdx.x] = 0; }
     if (threadIdx.x < 3) s_ends[threadIdx.x] = 0;
     if (threadIdx.x < ARC_MAX_BINS) s_esc[threadIdx.x] = 0.0;
@@ -300,9 +346,9 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                 const int ix = (int)fx, iy = (int)fy, iz = (int)fz;
                 ijk = (unsigned)ix | ((unsigned)iy << 10) | ((unsigned)iz << 20);
                 cell = (iz * N + iy) * N + ix;
-                if (dirx != 0.0) tx = __ddiv_rn(arc_sub((double)(ix + (dirx > 0.0)), gx), dirx);
-                if (diry != 0.0) ty = __ddiv_rn(arc_sub((double)(iy + (diry > 0.0)), gy), diry);
-                if (dirz != 0.0) tz = __ddiv_rn(arc_sub((double)(iz + (dirz > 0.0)), gz), dirz);
+                if (dirx != 0.0) { tx = __ddiv_rn(arc_sub((double)(ix + (dirx > 0.0)), gx), dirx); s_geo[6][threadIdx.x] = __ddiv_rn(1.0, dirx); }
+                if (diry != 0.0) { ty = __ddiv_rn(arc_sub((double)(iy + (diry > 0.0)), gy), diry); s_geo[7][threadIdx.x] = __ddiv_rn(1.0, diry); }
+                if (dirz != 0.0) { tz = __ddiv_rn(arc_sub((double)(iz + (dirz > 0.0)), gz), dirz); s_geo[8][threadIdx.x] = __ddiv_rn(1.0, dirz); }
             }
         }
 
@@ -327,7 +373,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
             const double r_out = split ? r_end : tmin;
             const double ds = arc_sub(r_out, r);
             const double dl = arc_mul(ds > 0.0 ? ds : 0.0, a.dx);
-            const double g_ax = s_geo[ax][threadIdx.x], d_ax = s_geo[3 + ax][threadIdx.x];
+            const double g_ax = s_geo[ax][threadIdx.x], d_ax = s_geo[3 + ax][threadIdx.x], y_ax = s_geo[6 + ax][threadIdx.x];
             const int pos = (__double2hiint(d_ax) >= 0) ? 1 : 0;          // d_ax > 0 (it is never zero on the crossed axis)
             const int st = 2 * pos - 1;
             const int sh = 10 * ax;
@@ -338,28 +384,34 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
             const bool go = !(split || out);
             KVec<KT, NB> knext;
             knext.load(kappa, go ? cell_next : cell);                       // always a valid cell: no divergence here
-            const double t_new = __ddiv_rn(arc_sub((double)(inext + pos), g_ax), d_ax);
+            const double t_new = arc_div_by_recip(arc_sub((double)(inext + pos), g_ax), d_ax, y_ax);   // == IEEE division (C3)
             // a7: optical depth (fp64, decides: contract C4) and the deposit of Eq. 1
             bool depleted = true;
             if constexpr (sizeof(KT) == 4) {
-                // fp32-field mode (tolerance 1e-3): the attenuation FACTOR is evaluated in fp32, everything that carries
-                // or decides stays fp64.  Thin segment: absorbed = P ome, kept = P - absorbed; thick: kept = P E,
-                // absorbed = P - kept - either way absorbed + kept = P exactly, and the small one is the accurate one.
+                // fp32-field mode (tolerance 1e-3): the attenuation FACTOR is evaluated in fp32, two bins per packed
+                // instruction (FMUL2 / FFMA2); everything that carries or decides stays fp64.  Thin segment (x < 1/64):
+                // absorbed = P ome with ome = x (1 - x/2 + x^2/6 - x^3/24) (truncation < 5e-10), kept = P - absorbed;
+                // otherwise kept = P E with E = 2^(-x log2 e) on the SFU, absorbed = P - kept (relative error of the
+                // absorbed part <= 64 x 2 ulp = 1.5e-5).  Either way absorbed + kept = P to fp64 rounding.
                 const float dlf = (float)dl;
+                float x[NBE], om[NBE], y[NBE];
+#pragma unroll
+                for (int v = 0; v < NBE; v += 2) {
+                    const unsigned long long xx = arc_mul2(arc_pack2(kcur.k[v], kcur.k[v + 1 < NB ? v + 1 : v]), arc_pack2(dlf, dlf));
+                    unsigned long long pp = arc_fma2(arc_pack2(-1.0f / 24.0f, -1.0f / 24.0f), xx, arc_pack2(1.0f / 6.0f, 1.0f / 6.0f));
+                    pp = arc_fma2(pp, xx, arc_pack2(-0.5f, -0.5f));
+                    pp = arc_fma2(pp, xx, arc_pack2(1.0f, 1.0f));
+                    pp = arc_mul2(pp, xx);
+                    const unsigned long long yy = arc_mul2(xx, arc_pack2(-1.4426950408889634f, -1.4426950408889634f));
+                    arc_unpack2(xx, x[v], x[v + 1]); arc_unpack2(pp, om[v], om[v + 1]); arc_unpack2(yy, y[v], y[v + 1]);
+                }
 #pragma unroll
                 for (int v = 0; v < NB; ++v) {
                     const double dtau = arc_mul(kcur.get(v), dl);
                     tau[v] = arc_add(tau[v], dtau);
                     depleted = depleted && (tau[v] >= a.tau_term);       // min_nu tau_nu >= tau_term
-                    const float x = kcur.k[v] * dlf;
-                    float p = 1.0f / 720.0f;                             // ome = x (1 - x/2 + x^2/6 - ... + x^5/720), x < 1/8
-                    p = fmaf(p, x, -1.0f / 120.0f);
-                    p = fmaf(p, x, 1.0f / 24.0f);
-                    p = fmaf(p, x, -1.0f / 6.0f);
-                    p = fmaf(p, x, 0.5f);
-                    p = fmaf(-p, x, 1.0f);
-                    const bool thin = x < 0.125f;
-                    const float f = thin ? p * x : arc_ex2(-1.4426950408889634f * x);
+                    const bool thin = x[v] < 0.015625f;
+                    const float f = thin ? om[v] : arc_ex2(y[v]);
                     const double q = P[v] * (double)f;
                     const double rest = P[v] - q;
                     av[v] = thin ? q : rest;
@@ -377,10 +429,6 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                     P[v] = P[v] * E;                            // photon conserving: the ray keeps P e^-dtau
                 }
             }
-            if (depleted) {
-#pragma unroll
-                for (int v = 0; v < NB; ++v) av[v] += P[v];     // reading G7: the remainder stays in this cell
-            }
             dcell = cell;
             ++nseg_b; ++nray_seg;
             if (FLAGS & FLAG_DIGEST) h = mix64(h ^ (unsigned long long)cell);
@@ -394,8 +442,11 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
             }
             if (depleted || !go || nray_seg > max_seg) {
                 active = false;
-                if (depleted) end = ARC_END_DEPLETED;
-                else if (split) end = ARC_END_SPLIT;
+                if (depleted) {
+                    end = ARC_END_DEPLETED;
+#pragma unroll
+                    for (int v = 0; v < NB; ++v) av[v] += P[v];     // reading G7: the remainder stays in this cell
+                } else if (split) end = ARC_END_SPLIT;
                 else {
                     if (!out) atomicCAS(&sc->error, 0, ARC_DEV_RAY_RUNAWAY);
 #pragma unroll
@@ -412,6 +463,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
           }
           // a7: deposit - the whole warp, converged
           if constexpr (DEP == DEP_AGG) {
+#if ARC_AGG_STEPS == 0
               // segmented sum over the lanes that share a cell, by pointer jumping along each group's lane list:
               // after ceil(log2(group size)) rounds the first lane of a group holds the group's sum
               const unsigned peers = __match_any_sync(0xffffffffu, dcell);
@@ -426,7 +478,24 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                   }
                   nxt = __shfl_sync(0xffffffffu, nxt, from);              // (a tail lane reads its own -1)
               }
-              if (lane == leader && dcell >= 0) {
+              const bool head = (lane == leader);
+#else
+              // lanes are ordered (family, child) in nested pixel order, so rays that share a cell sit in NEIGHBOURING
+              // lanes: sum over runs of equal cells (cut at multiples of 2^ARC_AGG_STEPS lanes) with a fixed number of
+              // shuffle-down steps; the first lane of a run issues the REDs.  Equal cells in non-adjacent lanes are
+              // simply deposited separately - the sums are the same.
+              const int prev = __shfl_up_sync(0xffffffffu, dcell, 1);
+              const bool head = (prev != dcell) || ((lane & ((1 << ARC_AGG_STEPS) - 1)) == 0);
+              const unsigned above = __ballot_sync(0xffffffffu, head) & (0xfffffffeu << lane);   // run heads after my lane
+              const int last = above ? __ffs(above) - 2 : 31;                                   // last lane of my run
+#pragma unroll
+              for (int d = 1; d < (1 << ARC_AGG_STEPS); d <<= 1) {
+                  const int take = lane + d <= last;
+#pragma unroll
+                  for (int v = 0; v < NB; ++v) arc_add_if(av[v], __shfl_down_sync(0xffffffffu, av[v], d), take);
+              }
+#endif
+              if (head && dcell >= 0) {
                   double *Ac = a.A + (long long)dcell * NBP;
 #pragma unroll
                   for (int v = 0; v < NB; ++v) arc_red_add(Ac + v, av[v]);
