@@ -39,9 +39,11 @@ enum { ARC_F32 = 0, ARC_F64 = 1 };                    /* dtype of the five gas f
 enum { ARC_HOST = 0, ARC_DEVICE = 1 };
 enum { ARC_OK = 0, ARC_EINVAL = -1, ARC_ENOMEM = -2, ARC_ECUDA = -3, ARC_ESTATE = -4, ARC_EOVERFLOW = -5 };
 enum { ARC_END_SPLIT = 0, ARC_END_DEPLETED = 1, ARC_END_ESCAPED = 2 };
-/* deposit routes of the tracer (same sums): every lane issues its own fp64 REDs, or lanes of a warp
- * that are in the same cell are summed in registers first and one lane issues the REDs.  AUTO = the faster one. */
-enum { ARC_DEPOSIT_AUTO = 0, ARC_DEPOSIT_RED = 1, ARC_DEPOSIT_AGG = 2 };
+/* deposit routes of the tracer (same sums): RED = every lane issues its own fp64 REDs; AGG = lanes of a
+ * warp that are in the same cell are summed in registers first and one lane issues the REDs; QUAD = a segment's bins are
+ * spread over the 4 lanes of a lane quad so that one RED instruction carries whole accumulator records.
+ * AUTO = the fastest measured for the bin count. */
+enum { ARC_DEPOSIT_AUTO = 0, ARC_DEPOSIT_RED = 1, ARC_DEPOSIT_AGG = 2, ARC_DEPOSIT_QUAD = 3 };
 
 /* Free parameters the paper names (PAPER.md:45 initial level, :96/:348 Phi, :154 eps; G7
  * tau_term) plus run-time switches of this implementation. */
@@ -60,7 +62,7 @@ typedef struct arc_params {
     int32_t digest;         /* 1: also accumulate the order-independent traversal digest (slower)    */
     int32_t async;          /* 1: arc_trace/arc_update_chemistry do not synchronise (see top)        */
     int32_t trace_blocks;   /* persistent-kernel grid size; 0 = SM count x resident blocks per SM    */
-    int32_t deposit;        /* how segments reach the accumulators: ARC_DEPOSIT_AUTO | _RED | _AGG                */
+    int32_t deposit;        /* how segments reach the accumulators: ARC_DEPOSIT_AUTO | _RED | _AGG | _QUAD        */
 } arc_params;
 
 /* Per-cell outputs of arc_trace (PAPER.md:83 Eq. 1, :134-138, :170): DEVICE pointers, N^3 doubles each. */

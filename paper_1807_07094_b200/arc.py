@@ -20,7 +20,7 @@ ARC_F32, ARC_F64 = 0, 1
 ARC_HOST, ARC_DEVICE = 0, 1
 ARC_OK, ARC_EINVAL, ARC_ENOMEM, ARC_ECUDA, ARC_ESTATE, ARC_EOVERFLOW = 0, -1, -2, -3, -4, -5
 ARC_END_SPLIT, ARC_END_DEPLETED, ARC_END_ESCAPED = 0, 1, 2
-ARC_DEPOSIT_AUTO, ARC_DEPOSIT_RED, ARC_DEPOSIT_AGG = 0, 1, 2
+ARC_DEPOSIT_AUTO, ARC_DEPOSIT_RED, ARC_DEPOSIT_AGG, ARC_DEPOSIT_QUAD = 0, 1, 2, 3
 ARC_MAX_BINS, ARC_MAX_LEVEL = 8, 16
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

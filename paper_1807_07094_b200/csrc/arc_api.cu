@@ -111,7 +111,7 @@ int arc_set_params(arc_ctx *c, const arc_params *p)
     if (!(p->eps_sub > 0.0)) return fail(c, ARC_EINVAL, "arc_set_params: eps_sub must be positive");
     if (!(p->x_floor >= 0.0 && p->x_floor < 1.0)) return fail(c, ARC_EINVAL, "arc_set_params: x_floor must be in [0, 1)");
     if (p->trace_blocks < 0) return fail(c, ARC_EINVAL, "arc_set_params: trace_blocks must be >= 0");
-    if (p->deposit < ARC_DEPOSIT_AUTO || p->deposit > ARC_DEPOSIT_AGG) return fail(c, ARC_EINVAL, "arc_set_params: bad deposit mode");
+    if (p->deposit < ARC_DEPOSIT_AUTO || p->deposit > ARC_DEPOSIT_QUAD) return fail(c, ARC_EINVAL, "arc_set_params: bad deposit mode");
     c->p = *p;
     c->have_rates = false;
     return ARC_OK;

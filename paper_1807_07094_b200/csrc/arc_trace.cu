@@ -37,11 +37,11 @@ __global__ void arc_pix2vec_kernel(const int32_t *level, const uint32_t *pix, in
 
 }  // namespace
 
-// ARC_DEPOSIT_* -> the kernel's DEP_* (1 RED, 2 AGG).  AUTO: see DESIGN.md 6.3 for the measurements behind it.
+// ARC_DEPOSIT_* -> the kernel's DEP_* (1 RED, 2 AGG, 3 T).  AUTO: see DESIGN.md 6.2 for the measurements behind it.
 int arc_trace_deposit_mode(const arc_ctx *c, int nb)
 {
-    (void)nb;
-    return c->p.deposit == ARC_DEPOSIT_RED ? 1 : 2;
+    if (c->p.deposit != ARC_DEPOSIT_AUTO) return c->p.deposit;
+    return nb >= 3 ? 3 : 2;
 }
 
 int arc_trace_occupancy_grid(arc_ctx *c, int nb, int flags)

@@ -33,10 +33,12 @@
 #define ARC_TRACE_MIN_BLOCKS 3     // resident blocks per SM the register budget is held to (<= 85 registers)
 #endif
 #ifndef ARC_AGG_STEPS
-#define ARC_AGG_STEPS 3            // warp-aggregated deposit: runs of up to 2^ARC_AGG_STEPS neighbouring lanes (0: match.any groups)
+#define ARC_AGG_STEPS 0            // warp-aggregated deposit: 0 = match.any groups (any lanes); k > 0 = runs of up to 2^k neighbouring lanes
 #endif
 #define DEP_RED 1           // every lane: nb fp64 REDs per segment
 #define DEP_AGG 2           // lanes of a warp that sit in the same cell are summed first (match.any + shuffles): one lane REDs
+#define DEP_T 3             // transposed: a cell's bins are spread over the 4 lanes of a lane quad (through shared memory), so
+                            // that ONE RED instruction carries whole accumulator records (L1 coalesces the quad's 4 doubles)
 
 namespace {
 
@@ -205,6 +207,22 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
     __shared__ unsigned long long s_splits[ARC_MAX_LEVEL], s_rays[ARC_MAX_LEVEL], s_ends[3];
     __shared__ double s_esc[ARC_MAX_BINS];
     __shared__ double s_geo[9][ARC_TRACE_THREADS];            // per thread: source position g[3], direction d[3], RN(1/d)[3]
+    // DEP_T staging: one row of NBP doubles per lane (each warp uses its own 32 rows, between __syncwarp()s only).
+    // NBP == 4: row r = 4q + k of quad q sits at row position r ^ (q & 3) with its two 16-byte halves swapped when q is
+    // odd, which makes both the 128-bit row stores and the quad-wise 64-bit reads of pass k bank-conflict free.
+    __shared__ __align__(1024) double s_dep[DEP == DEP_T ? ARC_TRACE_THREADS * NBP : 2];
+    [[maybe_unused]] unsigned dep_wr = 0, dep_rd = 0;         // shared-memory byte addresses: own row / pass 0 of my quad
+    if constexpr (DEP == DEP_T) {
+        const unsigned base = (unsigned)__cvta_generic_to_shared(s_dep) + (threadIdx.x & ~31u) * (NBP * 8u);
+        const unsigned q = lane >> 2, b = lane & 3;
+        if constexpr (NBP == 4) {
+            dep_wr = base + ((unsigned)lane ^ (q & 3u)) * 32u;
+            dep_rd = base + ((4u * q) ^ (q & 3u)) * 32u + ((((b >> 1) ^ q) & 1u) * 16u) + (b & 1u) * 8u;
+        } else {
+            dep_wr = base + (unsigned)lane * (NBP * 8u);
+            dep_rd = base + 4u * q * (NBP * 8u) + b * 8u;
+        }
+    }
     if (threadIdx.x < ARC_MAX_LEVEL) { s_splits[threadIdx.x] = 0; s_rays[threadIdx.x] = 0; }
     if (threadIdx.x < 3) s_ends[threadIdx.x] = 0;
     if (threadIdx.x < ARC_MAX_BINS) s_esc[threadIdx.x] = 0.0;
@@ -501,6 +519,56 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                   for (int v = 0; v < NB; ++v) arc_red_add(Ac + v, av[v]);
                   ++nred_b;
               }
+          } else if constexpr (DEP == DEP_T) {
+              // every lane stages its NB absorbed rates; then, in pass k = 0..3, the 4 lanes of quad q send the record of
+              // ray 4q + k: lane (q, b) issues bin b (and b + 4): the quad's REDs of one instruction fall in one 32-byte
+              // sector and leave the SM as one request - 2.5x the RED rate of one lane walking through the record
+              if constexpr (NBP == 4) {
+                  const bool odd = (lane >> 2) & 1;
+                  const double lo0 = odd ? av[NB > 2 ? 2 : 0] : av[0], lo1 = odd ? (NB > 3 ? av[3] : 0.0) : av[1];
+                  const double hi0 = odd ? av[0] : av[NB > 2 ? 2 : 0], hi1 = odd ? av[1] : (NB > 3 ? av[3] : 0.0);
+                  asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(dep_wr), "d"(lo0), "d"(lo1) : "memory");
+                  asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(dep_wr + 16u), "d"(hi0), "d"(hi1) : "memory");
+              } else {
+#pragma unroll
+                  for (int v = 0; v < NB; ++v) asm volatile("st.shared.f64 [%0], %1;" ::"r"(dep_wr + 8u * v), "d"(av[v]) : "memory");
+              }
+              __syncwarp();
+              // the quad's 4 rays are siblings (or 4 neighbouring root pixels) less than a cell apart: rays of the quad that
+              // sit in the same cell are summed first (pure ALU work: the cells and values are in registers anyway), so a
+              // cell gets one record per quad and iteration
+              int cq[4];
+              double vq[(NB + 3) / 4][4];
+#pragma unroll
+              for (int k = 0; k < 4; ++k) {
+                  cq[k] = __shfl_sync(0xffffffffu, dcell, (lane & ~3) + k);
+#pragma unroll
+                  for (int b0 = 0; b0 < NB; b0 += 4) {
+                      const unsigned ad = (NBP == 4) ? (dep_rd ^ (unsigned)(k << 5)) : (dep_rd + (unsigned)(k * NBP * 8 + b0 * 8));
+                      vq[b0 / 4][k] = 0.0;
+                      if (b0 + (lane & 3) < NB) asm volatile("ld.shared.f64 %0, [%1];" : "=d"(vq[b0 / 4][k]) : "r"(ad) : "memory");
+                  }
+              }
+#pragma unroll
+              for (int k = 0; k < 4; ++k) {
+                  bool first = cq[k] >= 0;                         // not merged into an earlier ray of the quad
+#pragma unroll
+                  for (int j = 0; j < k; ++j) first = first && (cq[j] != cq[k]);
+                  if (first) {
+                      double *Ac = a.A + (long long)cq[k] * NBP + (lane & 3);
+#pragma unroll
+                      for (int b0 = 0; b0 < NB; b0 += 4) {
+                          if (b0 + (lane & 3) < NB) {
+                              double v = vq[b0 / 4][k];
+#pragma unroll
+                              for (int j = k + 1; j < 4; ++j) if (cq[j] == cq[k]) v += vq[b0 / 4][j];
+                              arc_red_add(Ac + b0, v);
+                          }
+                      }
+                      if ((lane & 3) == 0) ++nred_b;
+                  }
+              }
+              __syncwarp();                       // rows are rewritten in the next iteration
           } else {
               if (dcell >= 0) {
                   double *Ac = a.A + (long long)dcell * NBP;
@@ -627,6 +695,7 @@ cudaError_t launch_nb(const TraceArgs &a, bool log, int dep, int grid, cudaStrea
 {
     switch (dep) {
         case DEP_AGG: return launch_dep<NB, KT, DEP_AGG>(a, log, grid, s);
+        case DEP_T: return launch_dep<NB, KT, DEP_T>(a, log, grid, s);
         default: return launch_dep<NB, KT, DEP_RED>(a, log, grid, s);
     }
 }
@@ -646,7 +715,7 @@ int occ_dep(int flags)
 template <int NB, typename KT>
 int occ_nb(int dep, int flags)
 {
-    return dep == DEP_AGG ? occ_dep<NB, KT, DEP_AGG>(flags) : occ_dep<NB, KT, DEP_RED>(flags);
+    return dep == DEP_AGG ? occ_dep<NB, KT, DEP_AGG>(flags) : dep == DEP_T ? occ_dep<NB, KT, DEP_T>(flags) : occ_dep<NB, KT, DEP_RED>(flags);
 }
 
 }  // namespace

@@ -67,7 +67,7 @@ def test_config1_per_ray_cell_sequences_bit_exact():
     (8, 2, 2, "f64", 0, 7), (8, 3, 1, "f32", 1, 8), (12, 2, 3, "f64", 1, 9), (16, 4, 4, "f32", 0, 10),
     (20, 3, 5, "f64", 2, 12), (9, 2, 8, "f32", 1, 13), (7, 5, 6, "f64", 0, 14), (13, 1, 7, "f64", 1, 15),
 ])
-@pytest.mark.parametrize("deposit", [arc.ARC_DEPOSIT_RED, arc.ARC_DEPOSIT_AGG])
+@pytest.mark.parametrize("deposit", [arc.ARC_DEPOSIT_RED, arc.ARC_DEPOSIT_AGG, arc.ARC_DEPOSIT_QUAD])
 def test_tiny_random_workloads_per_ray_and_rates(N, nsrc, nb, dtype, l0, seed, deposit):
     """off-centre sources at arbitrary positions, random fields, ragged sizes; every bin count 1..8 (odd counts
     exercise the padded accumulator record); every deposit route of the tracer"""
