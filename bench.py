@@ -61,6 +61,16 @@ def hbm_peak():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic(config: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one tracer launch on this workload, from the committed
+    `ncu --set full` capture (profiles/ncu_traffic.json names the capture); None if this workload has none."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f).get(config, {}).get("dram_bytes_per_launch")
+    except OSError:
+        return None
+
+
 def algorithmic_bytes_per_segment(w) -> int:
     """gather nb opacities at the field dtype + read-modify-write nb fp64 accumulators."""
     return (4 if w.dtype == "f32" else 8) * w.nb + 16 * w.nb
@@ -232,6 +242,14 @@ def run_cuda(args):
     cx.close()
     del dev_fields
 
+    # deposit records per segment: a statistic the production kernel does not count (digest builds do): one untimed trace
+    seg_per_record = None
+    if rank == 0:
+        with arc.Context(w, digest=1, stream=stream.cuda_stream, **extra) as cxd:
+            cxd.trace(0)
+            sd = cxd.stats()
+            seg_per_record = sd["segments"] / max(1, sd["deposit_records"])
+
     # ---- arm 2: end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     pin = [torch.from_numpy(np.ascontiguousarray(np.asarray(a, dtype=fdt))).pin_memory() for a in w.fields()]
     rates_host = [torch.empty(nc, dtype=torch.float64).pin_memory() for _ in range(4)]   # Gamma_HI, Gamma_HeI, Gamma_HeII, heat_total
@@ -282,7 +300,7 @@ def run_cuda(args):
             "gpu_launches": 5 * args.steps,
             "clocks": clocks,
             "roofline": {"bound": "hbm", "kernel": "arc_trace_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                         "frac": achieved / peak, "traffic": ncu_traffic(args.config), "peak_source": peak_src,
                          "algorithmic_bytes_per_segment": bytes_seg, "segments_per_launch": tot_seg / args.steps,
                          "kernel_ms_per_launch": kms / args.steps},
             "segments_per_step": [int(x) for x in seg_steps],
@@ -291,7 +309,7 @@ def run_cuda(args):
             "cell_updates_per_s": nc * args.steps / (sum(chem_ms) * 1e-3) if sum(chem_ms) > 0 else 0.0,
             "chem_subcycles_per_step": [int(x) for x in sub_steps],
             "photon_conservation_max_rel_err": conservation,
-            "segments_per_deposit_record": tot_seg / max(1.0, float(sum(rec_steps))),
+            "segments_per_deposit_record": seg_per_record,
             "host_wall_s": wall,
         }
         if world == 1 and not args.no_cpu_baseline:

@@ -59,6 +59,8 @@ static inline int arc_nbp(int nb) { return nb == 1 ? 1 : ((nb + 1) & ~1); }
 
 struct TraceArgs {
     int N, nb, l0, Lmax, nsrc;
+    int NN;                    // N * N (cell stride of a z step)
+    unsigned int max_seg;      // 3 N + 8: no ray has more segments (runaway guard)
     int nbp;                   // accumulator stride, arc_nbp(nb)
     double dx;                 // cell size [cm]
     double csplit;             // sqrt(3/(pi Phi)): split radius of level l = csplit * 2^l (cells)

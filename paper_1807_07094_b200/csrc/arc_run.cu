@@ -68,7 +68,7 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
 
     TraceArgs a;
     std::memset(&a, 0, sizeof(a));
-    a.N = c->N; a.nb = nb; a.nbp = arc_nbp(nb); a.l0 = c->p.l0; a.Lmax = c->p.Lmax; a.nsrc = c->nsrc;
+    a.N = c->N; a.NN = c->N * c->N; a.max_seg = 3u * (unsigned)c->N + 8u; a.nb = nb; a.nbp = arc_nbp(nb); a.l0 = c->p.l0; a.Lmax = c->p.Lmax; a.nsrc = c->nsrc;
     a.dx = c->dx;
     a.csplit = std::sqrt(3.0 / (3.14159265358979323846 * c->p.Phi));      // O2: r_split(l) = csplit 2^l cells
     a.tau_term = c->p.tau_term;

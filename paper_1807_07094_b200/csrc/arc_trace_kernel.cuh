@@ -207,22 +207,24 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
     __shared__ unsigned long long s_splits[ARC_MAX_LEVEL], s_rays[ARC_MAX_LEVEL], s_ends[3];
     __shared__ double s_esc[ARC_MAX_BINS];
     __shared__ double s_geo[9][ARC_TRACE_THREADS];            // per thread: source position g[3], direction d[3], RN(1/d)[3]
-    // DEP_T staging: one row of NBP doubles per lane (each warp uses its own 32 rows, between __syncwarp()s only).
-    // NBP == 4: row r = 4q + k of quad q sits at row position r ^ (q & 3) with its two 16-byte halves swapped when q is
-    // odd, which makes both the 128-bit row stores and the quad-wise 64-bit reads of pass k bank-conflict free.
-    __shared__ __align__(1024) double s_dep[DEP == DEP_T ? ARC_TRACE_THREADS * NBP : 2];
-    [[maybe_unused]] unsigned dep_wr = 0, dep_rd = 0;         // shared-memory byte addresses: own row / pass 0 of my quad
+    // DEP_T staging, per warp: NB planes of 32 doubles (plane = bin, column = lane), planes 33 doubles apart.  A lane
+    // stores its NB absorbed rates with NB 64-bit stores (consecutive lanes, consecutive words: conflict free); in pass k
+    // lane (quad q, b) reads column 4q + k of plane b: word 33 b + 4 q + k, i.e. bank pairs 2b + 8q (+ const) - all 16
+    // lanes of a half warp distinct.  Addresses are kept as two opaque registers (else ptxas re-derives them from
+    // %tid every iteration); bins and passes are immediate offsets.
+    constexpr int DEP_PLANE = 33 * 8;                         // bytes between planes
+    constexpr int DEP_WARP = ((NB * DEP_PLANE + 15) / 16) * 16;
+    __shared__ __align__(16) unsigned char s_dep[DEP == DEP_T ? ARC_WARPS_PER_BLOCK * DEP_WARP : 16];
+    [[maybe_unused]] unsigned dep_wr = 0, dep_rd = 0;         // shared-memory byte addresses: my column of plane 0 / column 4q of plane b
     if constexpr (DEP == DEP_T) {
-        const unsigned base = (unsigned)__cvta_generic_to_shared(s_dep) + (threadIdx.x & ~31u) * (NBP * 8u);
-        const unsigned q = lane >> 2, b = lane & 3;
-        if constexpr (NBP == 4) {
-            dep_wr = base + ((unsigned)lane ^ (q & 3u)) * 32u;
-            dep_rd = base + ((4u * q) ^ (q & 3u)) * 32u + ((((b >> 1) ^ q) & 1u) * 16u) + (b & 1u) * 8u;
-        } else {
-            dep_wr = base + (unsigned)lane * (NBP * 8u);
-            dep_rd = base + 4u * q * (NBP * 8u) + b * 8u;
-        }
+        const unsigned base = (unsigned)__cvta_generic_to_shared(s_dep) + (threadIdx.x >> 5) * DEP_WARP;
+        dep_wr = base + (unsigned)lane * 8u;
+        dep_rd = base + (unsigned)(lane & 3) * DEP_PLANE + (unsigned)(lane >> 2) * 32u;
+        asm volatile("" : "+r"(dep_wr), "+r"(dep_rd));
     }
+    // shared-memory byte address of s_geo[0][threadIdx.x] (opaque for the same reason); row stride ARC_TRACE_THREADS * 8
+    unsigned geo_ad = (unsigned)__cvta_generic_to_shared(&s_geo[0][threadIdx.x]);
+    asm volatile("" : "+r"(geo_ad));
     if (threadIdx.x < ARC_MAX_LEVEL) { s_splits[threadIdx.x] = 0; s_rays[threadIdx.x] = 0; }
     if (threadIdx.x < 3) s_ends[threadIdx.x] = 0;
     if (threadIdx.x < ARC_MAX_BINS) s_esc[threadIdx.x] = 0.0;
@@ -341,8 +343,9 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
             const double gx = __ldg(a.src_g + 3 * src), gy = __ldg(a.src_g + 3 * src + 1), gz = __ldg(a.src_g + 3 * src + 2);
             // the ray's constants live in shared memory (read back by this thread only: no barrier needed); the
             // loop fetches just the crossed axis' pair, which keeps 12 registers free for a third resident block
-            s_geo[0][threadIdx.x] = gx; s_geo[1][threadIdx.x] = gy; s_geo[2][threadIdx.x] = gz;
-            s_geo[3][threadIdx.x] = dirx; s_geo[4][threadIdx.x] = diry; s_geo[5][threadIdx.x] = dirz;
+            // (stores and loads of s_geo are volatile asm: kept in program order among themselves)
+#define GEO_ST(row, val) asm volatile("st.shared.f64 [%0+%1], %2;" ::"r"(geo_ad), "n"((row) * ARC_TRACE_THREADS * 8), "d"(val))
+            GEO_ST(0, gx); GEO_ST(1, gy); GEO_ST(2, gz); GEO_ST(3, dirx); GEO_ST(4, diry); GEO_ST(5, dirz);
             // split radii: exact power-of-two scalings of csplit (O2)
             r = (level == a.l0) ? 0.0 : scalbn(a.csplit, level - 1);
             r_end = (level >= a.Lmax) ? INF : scalbn(a.csplit, level);
@@ -364,9 +367,9 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                 const int ix = (int)fx, iy = (int)fy, iz = (int)fz;
                 ijk = (unsigned)ix | ((unsigned)iy << 10) | ((unsigned)iz << 20);
                 cell = (iz * N + iy) * N + ix;
-                if (dirx != 0.0) { tx = __ddiv_rn(arc_sub((double)(ix + (dirx > 0.0)), gx), dirx); s_geo[6][threadIdx.x] = __ddiv_rn(1.0, dirx); }
-                if (diry != 0.0) { ty = __ddiv_rn(arc_sub((double)(iy + (diry > 0.0)), gy), diry); s_geo[7][threadIdx.x] = __ddiv_rn(1.0, diry); }
-                if (dirz != 0.0) { tz = __ddiv_rn(arc_sub((double)(iz + (dirz > 0.0)), gz), dirz); s_geo[8][threadIdx.x] = __ddiv_rn(1.0, dirz); }
+                if (dirx != 0.0) { tx = __ddiv_rn(arc_sub((double)(ix + (dirx > 0.0)), gx), dirx); GEO_ST(6, __ddiv_rn(1.0, dirx)); }
+                if (diry != 0.0) { ty = __ddiv_rn(arc_sub((double)(iy + (diry > 0.0)), gy), diry); GEO_ST(7, __ddiv_rn(1.0, diry)); }
+                if (dirz != 0.0) { tz = __ddiv_rn(arc_sub((double)(iz + (dirz > 0.0)), gz), dirz); GEO_ST(8, __ddiv_rn(1.0, dirz)); }
             }
         }
 
@@ -374,8 +377,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
         // One warp iteration = one (ray, cell) segment per active lane.  Everything that is per axis is selected once
         // (the crossed axis), the advance costs one IEEE division, the next cell's opacities are requested before this
         // segment's attenuation arithmetic, and the state advance is unconditional (a lane that just ended is inactive).
-        const unsigned int max_seg = 3u * (unsigned)N + 8u;
-        unsigned int nray_seg = 0, nseg_b = 0, nred_b = 0;
+        unsigned int nseg_b = 0, nred_b = 0;     // (nseg_b also is this ray's segment count: one ray per lane and batch)
         KVec<KT, NB> kcur;
         kcur.load(kappa, cell);                 // (cell 0 for lanes without a ray: harmless)
         for (;;) {
@@ -389,19 +391,26 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
             if (tz < tmin) { tmin = tz; ax = 2; }
             const bool split = (r_end <= tmin);
             const double r_out = split ? r_end : tmin;
-            const double ds = arc_sub(r_out, r);
-            const double dl = arc_mul(ds > 0.0 ? ds : 0.0, a.dx);
-            const double g_ax = s_geo[ax][threadIdx.x], d_ax = s_geo[3 + ax][threadIdx.x], y_ax = s_geo[6 + ax][threadIdx.x];
+            double ds = arc_sub(r_out, r);
+            if (__double2hiint(ds) < 0) ds = 0.0;                          // max(ds, 0) (C4); ds is never NaN
+            const double dl = arc_mul(ds, a.dx);
+            double g_ax, d_ax, y_ax;
+            {
+                const unsigned ad = geo_ad + (unsigned)ax * (ARC_TRACE_THREADS * 8u);
+                asm volatile("ld.shared.f64 %0, [%1];" : "=d"(g_ax) : "r"(ad));
+                asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(d_ax) : "r"(ad), "n"(3 * ARC_TRACE_THREADS * 8));
+                asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(y_ax) : "r"(ad), "n"(6 * ARC_TRACE_THREADS * 8));
+            }
             const int pos = (__double2hiint(d_ax) >= 0) ? 1 : 0;          // d_ax > 0 (it is never zero on the crossed axis)
             const int st = 2 * pos - 1;
             const int sh = 10 * ax;
             const int inext = (int)((ijk >> sh) & 1023u) + st;
             const bool out = (unsigned)inext >= (unsigned)N;
-            const int stride = ax == 0 ? 1 : (ax == 1 ? N : N * N);
+            int stride = a.NN;
+            if (ax == 1) stride = N;
+            if (ax == 0) stride = 1;
             const int cell_next = cell + st * stride;
             const bool go = !(split || out);
-            KVec<KT, NB> knext;
-            knext.load(kappa, go ? cell_next : cell);                       // always a valid cell: no divergence here
             const double t_new = arc_div_by_recip(arc_sub((double)(inext + pos), g_ax), d_ax, y_ax);   // == IEEE division (C3)
             // a7: optical depth (fp64, decides: contract C4) and the deposit of Eq. 1
             bool depleted = true;
@@ -447,8 +456,11 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                     P[v] = P[v] * E;                            // photon conserving: the ray keeps P e^-dtau
                 }
             }
+            // the NEXT cell's opacities (always a valid cell: no divergence) go straight into kcur - its last use is above -
+            // and have the deposit stage plus the next march to arrive
+            kcur.load(kappa, go ? cell_next : cell);
             dcell = cell;
-            ++nseg_b; ++nray_seg;
+            ++nseg_b;
             if (FLAGS & FLAG_DIGEST) h = mix64(h ^ (unsigned long long)cell);
             if (FLAGS & FLAG_LOG) {
                 const unsigned long long e = atomicAdd(&sc->log_n, 1ull);
@@ -458,7 +470,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                 }
                 ++seq;
             }
-            if (depleted || !go || nray_seg > max_seg) {
+            if (depleted || !go || nseg_b > a.max_seg) {
                 active = false;
                 if (depleted) {
                     end = ARC_END_DEPLETED;
@@ -473,7 +485,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                 }
             }
             // unconditional advance
-            r = r_out; cell = cell_next; kcur = knext;
+            r = r_out; cell = cell_next;
             ijk += (unsigned)st << sh;
             tx = (ax == 0) ? t_new : tx;
             ty = (ax == 1) ? t_new : ty;
@@ -523,16 +535,8 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
               // every lane stages its NB absorbed rates; then, in pass k = 0..3, the 4 lanes of quad q send the record of
               // ray 4q + k: lane (q, b) issues bin b (and b + 4): the quad's REDs of one instruction fall in one 32-byte
               // sector and leave the SM as one request - 2.5x the RED rate of one lane walking through the record
-              if constexpr (NBP == 4) {
-                  const bool odd = (lane >> 2) & 1;
-                  const double lo0 = odd ? av[NB > 2 ? 2 : 0] : av[0], lo1 = odd ? (NB > 3 ? av[3] : 0.0) : av[1];
-                  const double hi0 = odd ? av[0] : av[NB > 2 ? 2 : 0], hi1 = odd ? av[1] : (NB > 3 ? av[3] : 0.0);
-                  asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(dep_wr), "d"(lo0), "d"(lo1) : "memory");
-                  asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(dep_wr + 16u), "d"(hi0), "d"(hi1) : "memory");
-              } else {
 #pragma unroll
-                  for (int v = 0; v < NB; ++v) asm volatile("st.shared.f64 [%0], %1;" ::"r"(dep_wr + 8u * v), "d"(av[v]) : "memory");
-              }
+              for (int v = 0; v < NB; ++v) asm volatile("st.shared.f64 [%0], %1;" ::"r"(dep_wr + (unsigned)(v * DEP_PLANE)), "d"(av[v]) : "memory");
               __syncwarp();
               // the quad's 4 rays are siblings (or 4 neighbouring root pixels) less than a cell apart: rays of the quad that
               // sit in the same cell are summed first (pure ALU work: the cells and values are in registers anyway), so a
@@ -544,9 +548,9 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                   cq[k] = __shfl_sync(0xffffffffu, dcell, (lane & ~3) + k);
 #pragma unroll
                   for (int b0 = 0; b0 < NB; b0 += 4) {
-                      const unsigned ad = (NBP == 4) ? (dep_rd ^ (unsigned)(k << 5)) : (dep_rd + (unsigned)(k * NBP * 8 + b0 * 8));
                       vq[b0 / 4][k] = 0.0;
-                      if (b0 + (lane & 3) < NB) asm volatile("ld.shared.f64 %0, [%1];" : "=d"(vq[b0 / 4][k]) : "r"(ad) : "memory");
+                      if (b0 + 4 <= NB || b0 + (lane & 3) < NB)
+                          asm volatile("ld.shared.f64 %0, [%1];" : "=d"(vq[b0 / 4][k]) : "r"(dep_rd + (unsigned)(b0 * DEP_PLANE + k * 8)) : "memory");
                   }
               }
 #pragma unroll
@@ -555,17 +559,19 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
 #pragma unroll
                   for (int j = 0; j < k; ++j) first = first && (cq[j] != cq[k]);
                   if (first) {
-                      double *Ac = a.A + (long long)cq[k] * NBP + (lane & 3);
+                      // record index in 32 bits where it fits (N <= 1024: cells < 2^30): one LEA + one wide multiply-add
+                      double *Ac = (NBP <= 4) ? a.A + ((unsigned)cq[k] * (unsigned)NBP + (unsigned)(lane & 3))
+                                              : a.A + (long long)cq[k] * NBP + (lane & 3);
 #pragma unroll
                       for (int b0 = 0; b0 < NB; b0 += 4) {
-                          if (b0 + (lane & 3) < NB) {
+                          if (b0 + 4 <= NB || b0 + (lane & 3) < NB) {
                               double v = vq[b0 / 4][k];
 #pragma unroll
                               for (int j = k + 1; j < 4; ++j) if (cq[j] == cq[k]) v += vq[b0 / 4][j];
                               arc_red_add(Ac + b0, v);
                           }
                       }
-                      if ((lane & 3) == 0) ++nred_b;
+                      if ((FLAGS & FLAG_DIGEST) && (lane & 3) == 0) ++nred_b;      // (statistic: digest builds only)
                   }
               }
               __syncwarp();                       // rows are rewritten in the next iteration
