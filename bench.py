@@ -200,6 +200,11 @@ def run_cuda(args):
         torch.cuda.synchronize()
 
     w = make_workload(args.config)
+    if args.sources:                      # profiling aid: the first K sources of the workload (named so in config.workload)
+        import dataclasses
+        K = min(args.sources, w.nsrc)
+        w = dataclasses.replace(w, name=f"{w.name}[first {K} sources]", src_pos_cm=w.src_pos_cm[:K], src_Ndot=w.src_Ndot[:K],
+                                src_binfrac=w.src_binfrac[:K])
     fdt = np.float32 if w.dtype == "f32" else np.float64
     tdt = torch.float32 if w.dtype == "f32" else torch.float64
     stream = torch.cuda.Stream()
@@ -330,6 +335,7 @@ def main():
     ap.add_argument("--config", default="config4")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sources", type=int, default=0, help="profiling aid: keep only the first K sources of the workload")
     ap.add_argument("--deposit", type=int, default=0, help="arc_params.deposit: 0 auto, 1 per-lane REDs, 2 warp-aggregated")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -71,6 +71,12 @@ __device__ __forceinline__ void arc_red_add(double *p, double v)
     asm volatile("red.relaxed.gpu.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
 }
 
+// the same under a predicate (@p REDG: no branch, no reconvergence barrier around it)
+__device__ __forceinline__ void arc_red_add_if(double *p, double v, bool take)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %2, 0;\n\t@p red.relaxed.gpu.global.add.f64 [%0], %1;\n\t}" ::"l"(p), "d"(v), "r"((int)take) : "memory");
+}
+
 // opacity gather: the NB opacities of one cell, kept at their storage type until used (fewer registers while
 // the prefetched copy is in flight); one vector load per cell where the layout allows
 template <typename KT, int NB> struct KVec;
@@ -204,7 +210,9 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
     constexpr int NBE = (NB + 1) & ~1;                        // bins rounded up to whole fp32 pairs
     unsigned long long nred = 0;                              // deposit records this lane sent to L2
 
-    __shared__ unsigned long long s_splits[ARC_MAX_LEVEL], s_rays[ARC_MAX_LEVEL], s_ends[3];
+    // per-block tallies: 32-bit shared atomics are native (64-bit ones are CAS loops); spilled to the 64-bit global
+    // counters at the end and whenever one passes 2^30 (tally_spill)
+    __shared__ unsigned int s_splits[ARC_MAX_LEVEL], s_rays[ARC_MAX_LEVEL], s_ends[3];
     __shared__ double s_esc[ARC_MAX_BINS];
     __shared__ double s_geo[9][ARC_TRACE_THREADS];            // per thread: source position g[3], direction d[3], RN(1/d)[3]
     // DEP_T staging, per warp: NB planes of 32 doubles (plane = bin, column = lane), planes 33 doubles apart.  A lane
@@ -213,8 +221,8 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
     // lanes of a half warp distinct.  Addresses are kept as two opaque registers (else ptxas re-derives them from
     // %tid every iteration); bins and passes are immediate offsets.
     constexpr int DEP_PLANE = 33 * 8;                         // bytes between planes
-    constexpr int DEP_WARP = ((NB * DEP_PLANE + 15) / 16) * 16;
-    __shared__ __align__(16) unsigned char s_dep[DEP == DEP_T ? ARC_WARPS_PER_BLOCK * DEP_WARP : 16];
+    constexpr int DEP_WARP = ((NB * DEP_PLANE + 255) / 256) * 256;     // 256-aligned warp regions: (dep_wr >> 3) & 31 is the lane
+    __shared__ __align__(256) unsigned char s_dep[DEP == DEP_T ? ARC_WARPS_PER_BLOCK * DEP_WARP : 16];
     [[maybe_unused]] unsigned dep_wr = 0, dep_rd = 0;         // shared-memory byte addresses: my column of plane 0 / column 4q of plane b
     if constexpr (DEP == DEP_T) {
         const unsigned base = (unsigned)__cvta_generic_to_shared(s_dep) + (threadIdx.x >> 5) * DEP_WARP;
@@ -358,11 +366,9 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
             const double dN = (double)N;
             const bool inside = fx >= 0.0 && fx < dN && fy >= 0.0 && fy < dN && fz >= 0.0 && fz < dN;
             if (FLAGS & FLAG_DIGEST) h = mix64(((unsigned long long)src << 40) | ((unsigned long long)level << 32) | pix);
-            atomicAdd(&s_rays[level], 1ull);
+            atomicAdd(&s_rays[level], 1u);
             if (!inside) {
-#pragma unroll
-                for (int v = 0; v < NB; ++v) atomicAdd(&s_esc[v], P[v]);
-                end = ARC_END_ESCAPED; active = false;
+                end = ARC_END_ESCAPED; active = false;          // (P goes to the escape tally after the loop)
             } else {
                 const int ix = (int)fx, iy = (int)fy, iz = (int)fz;
                 ijk = (unsigned)ix | ((unsigned)iy << 10) | ((unsigned)iz << 20);
@@ -479,9 +485,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                 } else if (split) end = ARC_END_SPLIT;
                 else {
                     if (!out) atomicCAS(&sc->error, 0, ARC_DEV_RAY_RUNAWAY);
-#pragma unroll
-                    for (int v = 0; v < NB; ++v) atomicAdd(&s_esc[v], P[v]);
-                    end = ARC_END_ESCAPED;
+                    end = ARC_END_ESCAPED;                      // what the ray still carries, P, leaves the box (a9): tallied after the loop
                 }
             }
             // unconditional advance
@@ -543,36 +547,40 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
               // cell gets one record per quad and iteration
               int cq[4];
               double vq[(NB + 3) / 4][4];
+              // lane and bin from the (live) staging address instead of %tid (an S2R per iteration otherwise)
+              const unsigned ln = (dep_wr >> 3) & 31u, bq = ln & 3u;
 #pragma unroll
               for (int k = 0; k < 4; ++k) {
-                  cq[k] = __shfl_sync(0xffffffffu, dcell, (lane & ~3) + k);
+                  cq[k] = __shfl_sync(0xffffffffu, dcell, (ln & ~3u) + k);
 #pragma unroll
                   for (int b0 = 0; b0 < NB; b0 += 4) {
                       vq[b0 / 4][k] = 0.0;
-                      if (b0 + 4 <= NB || b0 + (lane & 3) < NB)
+                      if (b0 + 4 <= NB || b0 + bq < NB)
                           asm volatile("ld.shared.f64 %0, [%1];" : "=d"(vq[b0 / 4][k]) : "r"(dep_rd + (unsigned)(b0 * DEP_PLANE + k * 8)) : "memory");
+                  }
+              }
+              // sums first (all lanes, no branches), then four predicated REDs
+              bool first[4];
+#pragma unroll
+              for (int k = 0; k < 4; ++k) {
+                  first[k] = cq[k] >= 0;                           // not merged into an earlier ray of the quad
+#pragma unroll
+                  for (int j = 0; j < k; ++j) first[k] = first[k] && (cq[j] != cq[k]);
+#pragma unroll
+                  for (int j = k + 1; j < 4; ++j) {
+                      const bool same = cq[j] == cq[k];
+#pragma unroll
+                      for (int b0 = 0; b0 < NB; b0 += 4) vq[b0 / 4][k] += same ? vq[b0 / 4][j] : 0.0;
                   }
               }
 #pragma unroll
               for (int k = 0; k < 4; ++k) {
-                  bool first = cq[k] >= 0;                         // not merged into an earlier ray of the quad
+                  // record index in 32 bits where it fits (N <= 1024: cells < 2^30): one LEA + one wide multiply-add
+                  double *Ac = (NBP <= 4) ? a.A + ((unsigned)cq[k] * (unsigned)NBP + bq) : a.A + (long long)cq[k] * NBP + bq;
 #pragma unroll
-                  for (int j = 0; j < k; ++j) first = first && (cq[j] != cq[k]);
-                  if (first) {
-                      // record index in 32 bits where it fits (N <= 1024: cells < 2^30): one LEA + one wide multiply-add
-                      double *Ac = (NBP <= 4) ? a.A + ((unsigned)cq[k] * (unsigned)NBP + (unsigned)(lane & 3))
-                                              : a.A + (long long)cq[k] * NBP + (lane & 3);
-#pragma unroll
-                      for (int b0 = 0; b0 < NB; b0 += 4) {
-                          if (b0 + 4 <= NB || b0 + (lane & 3) < NB) {
-                              double v = vq[b0 / 4][k];
-#pragma unroll
-                              for (int j = k + 1; j < 4; ++j) if (cq[j] == cq[k]) v += vq[b0 / 4][j];
-                              arc_red_add(Ac + b0, v);
-                          }
-                      }
-                      if ((FLAGS & FLAG_DIGEST) && (lane & 3) == 0) ++nred_b;      // (statistic: digest builds only)
-                  }
+                  for (int b0 = 0; b0 < NB; b0 += 4)
+                      arc_red_add_if(Ac + b0, vq[b0 / 4][k], first[k] && (b0 + 4 <= NB || b0 + bq < NB));
+                  if ((FLAGS & FLAG_DIGEST) && first[k] && bq == 0) ++nred_b;      // (statistic: digest builds only)
               }
               __syncwarp();                       // rows are rewritten in the next iteration
           } else {
@@ -588,8 +596,27 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
         __syncwarp();
 
         // ------------------------------------------------------------------ a8/a9: bookkeeping, push children
+        {
+            // a9 tallies, once per batch and warp: rays by end reason (ballots), photons that left the box (warp sum of P
+            // over the lanes whose ray escaped; P is untouched once a ray has ended)
+            const unsigned e0 = __ballot_sync(0xffffffffu, end == 0), e1 = __ballot_sync(0xffffffffu, end == 1), e2 = __ballot_sync(0xffffffffu, end == 2);
+            if (lane < 3) { const unsigned n = __popc(lane == 0 ? e0 : (lane == 1 ? e1 : e2)); if (n) atomicAdd(&s_ends[lane], n); }
+            if (e2) {
+#pragma unroll
+                for (int v = 0; v < NB; ++v) {
+                    double e = (end == ARC_END_ESCAPED) ? P[v] : 0.0;
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+                    if (lane == 0) atomicAdd(&s_esc[v], e);
+                }
+            }
+            if (lane < ARC_MAX_LEVEL) {                  // tally_spill: keep the 32-bit block tallies far from wrapping
+                if (s_rays[lane] > 0x40000000u) { const unsigned n = atomicExch(&s_rays[lane], 0u); atomicAdd(&a.stats->rays_level[lane], (unsigned long long)n); atomicAdd(&a.stats->rays, (unsigned long long)n); }
+                if (s_splits[lane] > 0x40000000u) atomicAdd(&a.stats->splits[lane], (unsigned long long)atomicExch(&s_splits[lane], 0u));
+                if (lane < 3 && s_ends[lane] > 0x40000000u) atomicAdd(&a.stats->ends[lane], (unsigned long long)atomicExch(&s_ends[lane], 0u));
+            }
+        }
         if (end >= 0) {
-            atomicAdd(&s_ends[end], 1ull);
             if (FLAGS & FLAG_DIGEST) { h = mix64(h ^ (0xE0ull + (unsigned long long)end)); digest += h; }
             if (FLAGS & FLAG_LOG) {
                 const unsigned long long e = atomicAdd(&sc->log_n, 1ull);
@@ -600,7 +627,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
             }
         }
         const bool do_split = (end == ARC_END_SPLIT);
-        if (do_split) atomicAdd(&s_splits[level], 1ull);
+        if (do_split) atomicAdd(&s_splits[level], 1u);
         const unsigned ballot = __ballot_sync(0xffffffffu, do_split);
         const int npush = __popc(ballot);
         if (top - bot + npush > ARC_STACK_CAP) {
@@ -680,10 +707,10 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
     }
     __syncthreads();
     if (threadIdx.x < ARC_MAX_LEVEL) {
-        if (s_splits[threadIdx.x]) atomicAdd(&a.stats->splits[threadIdx.x], s_splits[threadIdx.x]);
-        if (s_rays[threadIdx.x]) { atomicAdd(&a.stats->rays_level[threadIdx.x], s_rays[threadIdx.x]); atomicAdd(&a.stats->rays, s_rays[threadIdx.x]); }
+        if (s_splits[threadIdx.x]) atomicAdd(&a.stats->splits[threadIdx.x], (unsigned long long)s_splits[threadIdx.x]);
+        if (s_rays[threadIdx.x]) { atomicAdd(&a.stats->rays_level[threadIdx.x], (unsigned long long)s_rays[threadIdx.x]); atomicAdd(&a.stats->rays, (unsigned long long)s_rays[threadIdx.x]); }
     }
-    if (threadIdx.x < 3 && s_ends[threadIdx.x]) atomicAdd(&a.stats->ends[threadIdx.x], s_ends[threadIdx.x]);
+    if (threadIdx.x < 3 && s_ends[threadIdx.x]) atomicAdd(&a.stats->ends[threadIdx.x], (unsigned long long)s_ends[threadIdx.x]);
     if (threadIdx.x < NB && s_esc[threadIdx.x] != 0.0) atomicAdd(&a.stats->escaped[threadIdx.x], s_esc[threadIdx.x]);
 }
 
