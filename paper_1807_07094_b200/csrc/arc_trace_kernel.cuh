@@ -440,9 +440,14 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                 }
 #pragma unroll
                 for (int v = 0; v < NB; ++v) {
-                    const double dtau = arc_mul(kcur.get(v), dl);
-                    tau[v] = arc_add(tau[v], dtau);
+                    tau[v] = arc_add(tau[v], arc_mul(kcur.get(v), dl));
                     depleted = depleted && (tau[v] >= a.tau_term);       // min_nu tau_nu >= tau_term
+                }
+                // last use of kcur is above: the NEXT cell's opacities (always a valid cell: no divergence) go straight into
+                // it and have the rest of this iteration, the deposit stage and the next march to arrive
+                kcur.load(kappa, go ? cell_next : cell);
+#pragma unroll
+                for (int v = 0; v < NB; ++v) {
                     const bool thin = x[v] < 0.015625f;
                     const float f = thin ? om[v] : arc_ex2(y[v]);
                     const double q = P[v] * (double)f;
@@ -451,20 +456,22 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                     P[v] = thin ? rest : q;
                 }
             } else {
+                double dtau[NB];
 #pragma unroll
                 for (int v = 0; v < NB; ++v) {
-                    const double dtau = arc_mul(kcur.get(v), dl);
-                    tau[v] = arc_add(tau[v], dtau);
+                    dtau[v] = arc_mul(kcur.get(v), dl);
+                    tau[v] = arc_add(tau[v], dtau[v]);
                     depleted = depleted && (tau[v] >= a.tau_term);
+                }
+                kcur.load(kappa, go ? cell_next : cell);       // (as above)
+#pragma unroll
+                for (int v = 0; v < NB; ++v) {
                     double E, ome;
-                    arc_attenuate(dtau, E, ome);                // e^-dtau and 1 - e^-dtau
+                    arc_attenuate(dtau[v], E, ome);             // e^-dtau and 1 - e^-dtau
                     av[v] = P[v] * ome;                         // absorbed = P (1 - e^-dtau)
                     P[v] = P[v] * E;                            // photon conserving: the ray keeps P e^-dtau
                 }
             }
-            // the NEXT cell's opacities (always a valid cell: no divergence) go straight into kcur - its last use is above -
-            // and have the deposit stage plus the next march to arrive
-            kcur.load(kappa, go ? cell_next : cell);
             dcell = cell;
             ++nseg_b;
             if (FLAGS & FLAG_DIGEST) h = mix64(h ^ (unsigned long long)cell);
