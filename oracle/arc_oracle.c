@@ -51,6 +51,8 @@ typedef struct {
     int32_t max_subcycles;
     double eps_sub;           /* PAPER.md:154 */
     double x_floor;
+    int32_t geom_corr;        /* PAPER.md:100-114: 0 none, 1 f_c (Eq. 2), 2 f_c + secondary f'_c (Eq. 3), 3 f_c squared */
+    int32_t pad_;
 } orc_params;
 
 typedef struct {
@@ -292,11 +294,41 @@ int orc_trace(const orc_params *p, int nb, const double *kappa, int nsrc, const 
                     /* step 4: deposit (Eq. 1; reading G13: current rate S e^-tau) */
                     const int64_t c = ((int64_t)i[2] * N + i[1]) * N + i[0];
                     const double dl = ds * dx;
+                    /* geometric correction (Eq. 2-3; readings G25-G29).  D_edge: distance from the
+                     * midpoint of the segment to the nearest of the six cell faces; L_pix: width of the pixel at the
+                     * midpoint radius, r_mid sqrt(Omega_l); f_c = 1/2 + D_edge/L_pix if D_edge < L_pix/2, else 1. */
+                    double fc = 1.0; int64_t cn = -1;
+                    if (p->geom_corr) {
+                        const double rmid = 0.5 * (r + r_out);
+                        const double Lpix = rmid * ldexp(sqrt(ORC_PI / 3.0), -l);     /* sqrt(4 pi / (12 4^l)) = sqrt(pi/3) / 2^l */
+                        double D = INFINITY; int nax = 0, nside = 0;
+                        for (int a = 0; a < 3; ++a) {            /* faces in the order x-, x+, y-, y+, z-, z+; first minimum wins */
+                            const double m = g[a] + rmid * d[a];
+                            const double u = m - (double)i[a];
+                            const double hi = 1.0 - u;
+                            if (u < D) { D = u; nax = a; nside = -1; }
+                            if (hi < D) { D = hi; nax = a; nside = +1; }
+                        }
+                        if (D < 0.0) D = 0.0;                    /* (rounding can put the midpoint a hair outside) */
+                        if (2.0 * D < Lpix) {
+                            fc = 0.5 + D / Lpix;
+                            if (p->geom_corr == 3) fc = fc * fc;    /* Wise & Abel (2011) form */
+                            int j[3] = {i[0], i[1], i[2]};
+                            j[nax] += nside;
+                            if (j[nax] >= 0 && j[nax] < N) cn = ((int64_t)j[2] * N + j[1]) * N + j[0];
+                        }
+                    }
                     for (int v = 0; v < nb; ++v) {
                         const double dtau = kappa[c * nb + v] * dl;
                         const double a_v = S[v] * exp(-tau[v]) * (-expm1(-dtau));
-                        A[c * nb + v] += a_v;
-                        st->absorbed[v] += a_v;
+                        if (fc == 1.0) { A[c * nb + v] += a_v; st->absorbed[v] += a_v; }
+                        else {
+                            const double in = fc * a_v, off = a_v - in;          /* in + off = a_v */
+                            A[c * nb + v] += in; st->absorbed[v] += in;
+                            if (p->geom_corr == 2) {               /* Eq. 3: what f_c removed goes to the nearest adjacent cell */
+                                A[(cn >= 0 ? cn : c) * nb + v] += off; st->absorbed[v] += off;
+                            }
+                        }
                         tau[v] = tau[v] + dtau;
                     }
                     st->segments++;

@@ -32,7 +32,7 @@ class Params(C.Structure):
                 ("l0", C.c_int32), ("Lmax", C.c_int32), ("Phi", C.c_double), ("tau_term", C.c_double),
                 ("Yp", C.c_double), ("isothermal", C.c_int32), ("caseB", C.c_int32),
                 ("coll_ion", C.c_int32), ("max_subcycles", C.c_int32), ("eps_sub", C.c_double),
-                ("x_floor", C.c_double)]
+                ("x_floor", C.c_double), ("geom_corr", C.c_int32), ("pad_", C.c_int32)]
 
 
 class Stats(C.Structure):
@@ -84,7 +84,7 @@ def make_params(w, **override) -> Params:
                   Lmax=int(d["Lmax"]), Phi=float(d["Phi"]), tau_term=float(d["tau_term"]),
                   Yp=float(d["Yp"]), isothermal=int(d["isothermal"]), caseB=int(d["caseB"]),
                   coll_ion=int(d["coll_ion"]), max_subcycles=int(d["max_subcycles"]),
-                  eps_sub=float(d["eps_sub"]), x_floor=float(d["x_floor"]))
+                  eps_sub=float(d["eps_sub"]), x_floor=float(d["x_floor"]), geom_corr=int(d.get("geom_corr", 0)))
 
 
 # ---- O1/O2 -------------------------------------------------------------------------------
