@@ -44,6 +44,12 @@ enum { ARC_END_SPLIT = 0, ARC_END_DEPLETED = 1, ARC_END_ESCAPED = 2 };
  * spread over the 4 lanes of a lane quad so that one RED instruction carries whole accumulator records.
  * AUTO = the fastest measured for the bin count. */
 enum { ARC_DEPOSIT_AUTO = 0, ARC_DEPOSIT_RED = 1, ARC_DEPOSIT_AGG = 2, ARC_DEPOSIT_QUAD = 3 };
+/* geometric correction of the deposit (Eq. 2-3, study at :338-354; readings G25-G29):
+ * NONE; FC = each segment's absorbed rate times f_c = 1/2 + D_edge/L_pix (capped at 1), the rest is lost; FC_SECONDARY =
+ * the paper's choice: what f_c removed goes to the adjacent cell across the nearest face (photon conserving; kept in the
+ * cell when that neighbour is outside the box); FC2 = f_c squared (Wise & Abel 2011), the rest lost.  The ray itself
+ * (optical depth, splitting, termination) is the same in every mode. */
+enum { ARC_GEOM_NONE = 0, ARC_GEOM_FC = 1, ARC_GEOM_FC_SECONDARY = 2, ARC_GEOM_FC2 = 3 };
 
 /* Free parameters the paper names (PAPER.md:45 initial level, :96/:348 Phi, :154 eps; G7
  * tau_term) plus run-time switches of this implementation. */
@@ -63,6 +69,8 @@ typedef struct arc_params {
     int32_t async;          /* 1: arc_trace/arc_update_chemistry do not synchronise (see top)        */
     int32_t trace_blocks;   /* persistent-kernel grid size; 0 = SM count x resident blocks per SM    */
     int32_t deposit;        /* how segments reach the accumulators: ARC_DEPOSIT_AUTO | _RED | _AGG | _QUAD        */
+    int32_t geom_corr;      /* ARC_GEOM_NONE | _FC | _FC_SECONDARY | _FC2; needs deposit = AUTO */
+    int32_t reserved0;      /* keep 0                                                                 */
 } arc_params;
 
 /* Per-cell outputs of arc_trace (PAPER.md:83 Eq. 1, :134-138, :170): DEVICE pointers, N^3 doubles each. */

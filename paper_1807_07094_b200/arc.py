@@ -21,6 +21,7 @@ ARC_HOST, ARC_DEVICE = 0, 1
 ARC_OK, ARC_EINVAL, ARC_ENOMEM, ARC_ECUDA, ARC_ESTATE, ARC_EOVERFLOW = 0, -1, -2, -3, -4, -5
 ARC_END_SPLIT, ARC_END_DEPLETED, ARC_END_ESCAPED = 0, 1, 2
 ARC_DEPOSIT_AUTO, ARC_DEPOSIT_RED, ARC_DEPOSIT_AGG, ARC_DEPOSIT_QUAD = 0, 1, 2, 3
+ARC_GEOM_NONE, ARC_GEOM_FC, ARC_GEOM_FC_SECONDARY, ARC_GEOM_FC2 = 0, 1, 2, 3
 ARC_MAX_BINS, ARC_MAX_LEVEL = 8, 16
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -42,7 +43,8 @@ class arc_params(C.Structure):
     _fields_ = [("l0", C.c_int32), ("Lmax", C.c_int32), ("Phi", C.c_double), ("tau_term", C.c_double),
                 ("Yp", C.c_double), ("isothermal", C.c_int32), ("caseB", C.c_int32), ("coll_ion", C.c_int32),
                 ("max_subcycles", C.c_int32), ("eps_sub", C.c_double), ("x_floor", C.c_double),
-                ("digest", C.c_int32), ("async_", C.c_int32), ("trace_blocks", C.c_int32), ("deposit", C.c_int32)]
+                ("digest", C.c_int32), ("async_", C.c_int32), ("trace_blocks", C.c_int32), ("deposit", C.c_int32),
+                ("geom_corr", C.c_int32), ("reserved0", C.c_int32)]
 
 
 class arc_rates(C.Structure):

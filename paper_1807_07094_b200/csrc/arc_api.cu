@@ -37,7 +37,7 @@ void arc_default_params(arc_params *p)
     std::memset(p, 0, sizeof(*p));
     p->l0 = 1; p->Lmax = 13; p->Phi = 3.0; p->tau_term = 30.0; p->Yp = 0.0;
     p->isothermal = 1; p->caseB = 1; p->coll_ion = 0; p->max_subcycles = 4096;
-    p->eps_sub = 0.1; p->x_floor = 1e-12; p->digest = 0; p->async = 0; p->trace_blocks = 0; p->deposit = ARC_DEPOSIT_AUTO;
+    p->eps_sub = 0.1; p->x_floor = 1e-12; p->digest = 0; p->async = 0; p->trace_blocks = 0; p->deposit = ARC_DEPOSIT_AUTO; p->geom_corr = ARC_GEOM_NONE; p->reserved0 = 0;
 }
 
 int arc_create_grid(arc_ctx **out, int N, double box_cm, int dtype)
@@ -112,6 +112,9 @@ int arc_set_params(arc_ctx *c, const arc_params *p)
     if (!(p->x_floor >= 0.0 && p->x_floor < 1.0)) return fail(c, ARC_EINVAL, "arc_set_params: x_floor must be in [0, 1)");
     if (p->trace_blocks < 0) return fail(c, ARC_EINVAL, "arc_set_params: trace_blocks must be >= 0");
     if (p->deposit < ARC_DEPOSIT_AUTO || p->deposit > ARC_DEPOSIT_QUAD) return fail(c, ARC_EINVAL, "arc_set_params: bad deposit mode");
+    if (p->geom_corr < ARC_GEOM_NONE || p->geom_corr > ARC_GEOM_FC2) return fail(c, ARC_EINVAL, "arc_set_params: bad geom_corr");
+    if (p->geom_corr != ARC_GEOM_NONE && p->deposit != ARC_DEPOSIT_AUTO)
+        return fail(c, ARC_EINVAL, "arc_set_params: the geometric correction is built for deposit = ARC_DEPOSIT_AUTO only");
     c->p = *p;
     c->have_rates = false;
     return ARC_OK;

@@ -65,6 +65,8 @@ struct TraceArgs {
     double dx;                 // cell size [cm]
     double csplit;             // sqrt(3/(pi Phi)): split radius of level l = csplit * 2^l (cells)
     double tau_term;
+    double cpix;               // sqrt(pi/3): pixel width of level l at radius r is r cpix 2^-l (geometric correction)
+    int geom;                  // ARC_GEOM_*
     const void *kappa;         // [cell][nb] at field dtype
     double *A;                 // [cell][nbp] absorbed photons/s (entries nb..nbp-1 stay zero)
     const double *src_g;       // [nsrc][3] source position in grid units

@@ -28,6 +28,7 @@
 
 #define FLAG_LOG 1          // template flag: per-ray logging (arc_trace_debug)
 #define FLAG_DIGEST 2       // template flag: accumulate the order-independent traversal digest
+#define FLAG_GEOM 4         // template flag: geometric correction of the deposit (Eq. 2-3), mode in TraceArgs::geom
 
 #ifndef ARC_TRACE_MIN_BLOCKS
 #define ARC_TRACE_MIN_BLOCKS 3     // resident blocks per SM the register budget is held to (<= 85 registers)
@@ -390,6 +391,8 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
           if (!__any_sync(0xffffffffu, active)) break;
           double av[NB];
           int dcell = -1 - lane;                 // deposit key; lanes without a segment keep a unique negative one
+          [[maybe_unused]] double avn[NB];       // FLAG_GEOM: what Eq. 3 hands to the adjacent cell ...
+          [[maybe_unused]] int ncell = -1 - lane;  // ... and that cell (same convention as dcell)
           if (active) {
             // a6: first face crossed; ties go to x, then y (reading G9)
             int ax = 0; double tmin = tx;
@@ -472,6 +475,44 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                     P[v] = P[v] * E;                            // photon conserving: the ray keeps P e^-dtau
                 }
             }
+            if constexpr ((FLAGS & FLAG_GEOM) != 0) {
+                // Geometric correction (readings G25-G29).  Which face is nearest decides where photons
+                // go, so that part is contract arithmetic (explicit round-to-nearest operations in the oracle's order):
+                // midpoint m_a = g_a + r_mid d_a, u_a = m_a - i_a, faces in the order x-, x+, y-, y+, z-, z+, first
+                // minimum wins; D_edge = max(min, 0); L_pix = r_mid (cpix 2^-l); f_c = 1/2 + D_edge / L_pix if
+                // 2 D_edge < L_pix, else 1.  The ray's own tau and P are not touched.
+                const double rmid = arc_mul(0.5, arc_add(r, r_out));
+                const double Lpix = arc_mul(rmid, scalbn(a.cpix, -level));
+                double D = INF; int nax = 0, nside = 0;
+#pragma unroll
+                for (int ax3 = 0; ax3 < 3; ++ax3) {
+                    double g3, d3;
+                    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(g3) : "r"(geo_ad + (unsigned)(ax3 * ARC_TRACE_THREADS * 8)));
+                    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(d3) : "r"(geo_ad + (unsigned)((3 + ax3) * ARC_TRACE_THREADS * 8)));
+                    const double u = arc_sub(arc_add(g3, arc_mul(rmid, d3)), (double)((ijk >> (10 * ax3)) & 1023u));
+                    const double hi = arc_sub(1.0, u);
+                    if (u < D) { D = u; nax = ax3; nside = -1; }
+                    if (hi < D) { D = hi; nax = ax3; nside = 1; }
+                }
+                if (D < 0.0) D = 0.0;
+                ncell = -1 - lane;
+                if (arc_mul(2.0, D) < Lpix) {
+                    double fc = arc_add(0.5, __ddiv_rn(D, Lpix));
+                    if (a.geom == ARC_GEOM_FC2) fc = arc_mul(fc, fc);
+                    const int jn = (int)((ijk >> (10 * nax)) & 1023u) + nside;
+                    const bool nb_in = (unsigned)jn < (unsigned)N;
+                    const int nstride = nax == 0 ? 1 : (nax == 1 ? N : a.NN);
+                    const bool move = (a.geom == ARC_GEOM_FC_SECONDARY) && nb_in;
+                    if (move) ncell = cell + nside * nstride;
+#pragma unroll
+                    for (int v = 0; v < NB; ++v) {
+                        const double in = fc * av[v], off = av[v] - in;
+                        avn[v] = off;                                         // (read only where ncell >= 0)
+                        // secondary correction with the neighbour outside the box: the cell keeps everything (G29)
+                        av[v] = (a.geom == ARC_GEOM_FC_SECONDARY && !nb_in) ? av[v] : in;
+                    }
+                }
+            }
             dcell = cell;
             ++nseg_b;
             if (FLAGS & FLAG_DIGEST) h = mix64(h ^ (unsigned long long)cell);
@@ -502,7 +543,8 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
             ty = (ax == 1) ? t_new : ty;
             tz = (ax == 2) ? t_new : tz;
           }
-          // a7: deposit - the whole warp, converged
+          // a7: deposit - the whole warp, converged (a lambda: the geometric correction runs the stage a second time)
+          auto deposit = [&](const int dcell, double (&av)[NB]) {
           if constexpr (DEP == DEP_AGG) {
 #if ARC_AGG_STEPS == 0
               // segmented sum over the lanes that share a cell, by pointer jumping along each group's lane list:
@@ -597,6 +639,11 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                   for (int v = 0; v < NB; ++v) arc_red_add(Ac + v, av[v]);   // a7: REDG.E.ADD.F64 ("atomically")
                   ++nred_b;
               }
+          }
+          };
+          deposit(dcell, av);
+          if constexpr ((FLAGS & FLAG_GEOM) != 0) {
+              if (__any_sync(0xffffffffu, ncell >= 0)) deposit(ncell, avn);        // Eq. 3: the adjacent cells' share
           }
         }
         nseg += nseg_b; nred += nred_b;
@@ -724,6 +771,14 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
 template <int NB, typename KT, int DEP>
 cudaError_t launch_dep(const TraceArgs &a, bool log, int grid, cudaStream_t s)
 {
+    if (a.flags & FLAG_GEOM) {                   // built for the AUTO deposit route of this bin count only (arc_set_params checks)
+        if constexpr (DEP == (NB >= 3 ? DEP_T : DEP_AGG)) {
+            if (log) arc_trace_kernel<NB, KT, FLAG_GEOM | FLAG_LOG | FLAG_DIGEST, DEP><<<grid, ARC_TRACE_THREADS, 0, s>>>(a);
+            else if (a.flags & FLAG_DIGEST) arc_trace_kernel<NB, KT, FLAG_GEOM | FLAG_DIGEST, DEP><<<grid, ARC_TRACE_THREADS, 0, s>>>(a);
+            else arc_trace_kernel<NB, KT, FLAG_GEOM, DEP><<<grid, ARC_TRACE_THREADS, 0, s>>>(a);
+            return cudaGetLastError();
+        } else return cudaErrorInvalidValue;
+    }
     if (log) arc_trace_kernel<NB, KT, FLAG_LOG | FLAG_DIGEST, DEP><<<grid, ARC_TRACE_THREADS, 0, s>>>(a);
     else if (a.flags & FLAG_DIGEST) arc_trace_kernel<NB, KT, FLAG_DIGEST, DEP><<<grid, ARC_TRACE_THREADS, 0, s>>>(a);
     else arc_trace_kernel<NB, KT, 0, DEP><<<grid, ARC_TRACE_THREADS, 0, s>>>(a);
@@ -745,6 +800,15 @@ int occ_dep(int flags)
 {
     int nblk = 0;
     cudaError_t e;
+    if (flags & FLAG_GEOM) {
+        if constexpr (DEP == (NB >= 3 ? DEP_T : DEP_AGG)) {
+            if (flags & FLAG_LOG) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, arc_trace_kernel<NB, KT, FLAG_GEOM | FLAG_LOG | FLAG_DIGEST, DEP>, ARC_TRACE_THREADS, 0);
+            else if (flags & FLAG_DIGEST) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, arc_trace_kernel<NB, KT, FLAG_GEOM | FLAG_DIGEST, DEP>, ARC_TRACE_THREADS, 0);
+            else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, arc_trace_kernel<NB, KT, FLAG_GEOM, DEP>, ARC_TRACE_THREADS, 0);
+        } else e = cudaErrorInvalidValue;
+        if (e != cudaSuccess) { cudaGetLastError(); return 1; }
+        return nblk < 1 ? 1 : nblk;
+    }
     if (flags & FLAG_LOG) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, arc_trace_kernel<NB, KT, FLAG_LOG | FLAG_DIGEST, DEP>, ARC_TRACE_THREADS, 0);
     else if (flags & FLAG_DIGEST) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, arc_trace_kernel<NB, KT, FLAG_DIGEST, DEP>, ARC_TRACE_THREADS, 0);
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, arc_trace_kernel<NB, KT, 0, DEP>, ARC_TRACE_THREADS, 0);
