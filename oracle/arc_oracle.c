@@ -550,5 +550,43 @@ int64_t orc_chemistry(const orc_params *p, const double *nH, double *xHI, double
     return total;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * Radiative-transfer time step (readings G30-G31).  Per cell, with the rates of the
+ * last trace and the current fields: dn_HI/dt = n_H (D - C x_HI) with Eq. 4's D = alpha_HII n_e x_HII,
+ * C = Gamma_HI + C_HI n_e.  scheme 1 (:182-190): dt_n = eps n_HI / |dn_HI/dt| over the cells with
+ * tau = n_HI sigma_1 d > 0.5; scheme 2 (:192-204): dt_I = eps / (sigma_1 d |dn_HI/dt|) over all cells.  Returns the
+ * minimum (+inf if no cell qualifies or nothing changes); *n_used = cells that entered the minimum.
+ * ------------------------------------------------------------------------------------------ */
+double orc_suggest_dt(const orc_params *p, int scheme, double eps, double sigma1, const double *nH, const double *xHI,
+                      const double *xHeI, const double *xHeII, const double *T, const double *GammaHI, int64_t *n_used)
+{
+    const int64_t nc = (int64_t)p->N * p->N * p->N;
+    const double d = p->box_cm / (double)p->N;
+    double best = INFINITY;
+    int64_t used = 0;
+    for (int64_t c = 0; c < nc; ++c) {
+        const double nHe = n_He_of(nH[c], p->Yp);
+        const double xHII = 1.0 - xHI[c];
+        double xHeIII = 1.0 - xHeI[c] - xHeII[c]; if (xHeIII < 0.0) xHeIII = 0.0;
+        const double ne = nH[c] * xHII + nHe * (xHeII[c] + 2.0 * xHeIII);
+        double co[15];
+        orc_rate_coeffs(T[c], p->caseB, p->coll_ion, co);
+        const double C0 = GammaHI[c] + co[3] * ne, D0 = co[0] * ne * xHII;
+        const double nHI = nH[c] * xHI[c];
+        const double ndot = fabs(nH[c] * (D0 - C0 * xHI[c]));
+        if (ndot == 0.0) continue;
+        double dt;
+        if (scheme == 1) {
+            const double tau = (nHI * sigma1) * d;
+            if (!(tau > 0.5)) continue;
+            dt = eps * nHI / ndot;
+        } else dt = eps / ((sigma1 * d) * ndot);
+        ++used;
+        if (dt < best) best = dt;
+    }
+    if (n_used) *n_used = used;
+    return best;
+}
+
 int orc_sizeof_params(void) { return (int)sizeof(orc_params); }
 int orc_sizeof_stats(void) { return (int)sizeof(orc_stats); }

@@ -213,6 +213,20 @@ def chem_cell(w_or_params, nH, x, T, G, H, dt):
     return xx, float(TT[0]), int(k)
 
 
+def suggest_dt(w, fields, GammaHI, scheme=1, eps=0.1, **override):
+    """Radiative-transfer time step: scheme 1 = neutral-fraction change in cells with tau > 0.5,
+    scheme 2 = intensity change.  -> (dt_s, cells that entered the minimum)."""
+    p = make_params(w, **override)
+    nH, xHI, xHeI, xHeII, T = [_f64(a) for a in fields]
+    used = C.c_int64(0)
+    l = lib()
+    l.orc_suggest_dt.restype = C.c_double
+    l.orc_suggest_dt.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double] + [C.c_void_p] * 7
+    dt = l.orc_suggest_dt(C.byref(p), int(scheme), float(eps), float(w.sig_HI[0]), _p(nH), _p(xHI), _p(xHeI), _p(xHeII),
+                          _p(T), _p(_f64(GammaHI)), C.byref(used))
+    return float(dt), int(used.value)
+
+
 def step(w, fields, dt=None, **override):
     """One full hot-path pass: opacity -> trace -> finalize -> chemistry.  -> dict."""
     kappa = opacity(w, fields, **override)
