@@ -160,6 +160,16 @@ int arc_get_accum(arc_ctx *c, double *A, int where);
  * trace has been done since the fields were last set. */
 int arc_update_chemistry(arc_ctx *c, double dt_s);
 
+/* Radiative-transfer time step, from the CURRENT fields and the rates of the last arc_trace:
+ * per cell dn_HI/dt = n_H (alpha_HII n_e x_HII - (Gamma_HI + C_HI n_e) x_HI) (Eq. 4);
+ *   scheme ARC_DT_NEUTRAL   (i):  min over cells with tau = n_HI sigma_1 d > 0.5 of eps n_HI / |dn_HI/dt|   (:182-190)
+ *   scheme ARC_DT_INTENSITY (ii): min over all cells of eps / (sigma_1 d |dn_HI/dt|)                         (:192-204)
+ * sigma_1 = H I cross-section of the first (softest) bin, d = cell width.  *dt_s = +inf if no cell qualifies;
+ * *cells_used (may be NULL) = cells that entered the minimum.  One streaming reduction kernel; synchronises.
+ * ARC_ESTATE without valid rates. */
+enum { ARC_DT_NEUTRAL = 1, ARC_DT_INTENSITY = 2 };
+int arc_suggest_dt(arc_ctx *c, int scheme, double eps, double *dt_s, int64_t *cells_used);
+
 int arc_synchronize(arc_ctx *c);                       /* wait for the stream; report deferred errors */
 int arc_get_stats(arc_ctx *c, arc_stats *s);           /* synchronises */
 

@@ -29,7 +29,7 @@ LIB_PATH = os.path.join(_HERE, "libarc_b200.so")
 
 EXPORTS = ["arc_create_grid", "arc_destroy", "arc_default_params", "arc_set_params", "arc_set_stream",
            "arc_set_fields", "arc_get_fields", "arc_set_spectrum", "arc_set_sources", "arc_trace",
-           "arc_get_rates", "arc_get_accum", "arc_update_chemistry", "arc_synchronize", "arc_get_stats",
+           "arc_get_rates", "arc_get_accum", "arc_update_chemistry", "arc_suggest_dt", "arc_synchronize", "arc_get_stats",
            "arc_trace_debug", "arc_pix2vec", "arc_last_error", "arc_version"]
 
 
@@ -94,6 +94,7 @@ def lib():
         l.arc_get_rates.argtypes = [vp] + [vp] * 7 + [i32]
         l.arc_get_accum.argtypes = [vp, vp, i32]
         l.arc_update_chemistry.argtypes = [vp, dbl]
+        l.arc_suggest_dt.argtypes = [vp, i32, dbl, vp, vp]
         l.arc_synchronize.argtypes = [vp]
         l.arc_get_stats.argtypes = [vp, C.POINTER(arc_stats)]
         l.arc_trace_debug.argtypes = [vp, i32, C.POINTER(arc_raylog)]
@@ -219,6 +220,17 @@ def arc_update_chemistry(ctx, dt_s: float):
     return _check(ctx, lib().arc_update_chemistry(ctx, float(dt_s)))
 
 
+ARC_DT_NEUTRAL, ARC_DT_INTENSITY = 1, 2
+
+
+def arc_suggest_dt(ctx, scheme: int = ARC_DT_NEUTRAL, eps: float = 0.1):
+    """-> (dt_s, cells that entered the minimum)."""
+    dt = C.c_double(0.0)
+    used = C.c_int64(0)
+    _check(ctx, lib().arc_suggest_dt(ctx, int(scheme), float(eps), C.byref(dt), C.byref(used)))
+    return float(dt.value), int(used.value)
+
+
 def arc_synchronize(ctx):
     return _check(ctx, lib().arc_synchronize(ctx))
 
@@ -327,6 +339,9 @@ class Context:
         A = np.zeros((self.w.ncell, self.nb))
         arc_get_accum(self.ctx, A)
         return A
+
+    def suggest_dt(self, scheme=ARC_DT_NEUTRAL, eps=0.1):
+        return arc_suggest_dt(self.ctx, scheme, eps)
 
     def update_chemistry(self, dt=None):
         return arc_update_chemistry(self.ctx, self.w.dt_s if dt is None else dt)

@@ -91,7 +91,7 @@ int arc_destroy(arc_ctx *c)
     if (!c) return ARC_OK;
     cudaStreamSynchronize(c->stream);
     for (int i = 0; i < 5; ++i) cudaFree(c->f[i]);
-    cudaFree(c->d_rates); cudaFree(c->d_sched); cudaFree(c->d_stats); cudaFree(c->d_absorbed);
+    cudaFree(c->d_rates); cudaFree(c->d_sched); cudaFree(c->d_stats); cudaFree(c->d_absorbed); cudaFree(c->d_dt);
     cudaFree(c->d_kappa); cudaFree(c->d_A); cudaFree(c->d_src_g); cudaFree(c->d_src_S);
     cudaFree(c->d_stacks); cudaFree(c->d_queue); cudaFree(c->d_qseq);
     for (int i = 0; i < 8; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);

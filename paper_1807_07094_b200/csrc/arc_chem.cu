@@ -141,6 +141,60 @@ __global__ void __launch_bounds__(128) arc_chem_kernel(long long ncell, double d
     if ((threadIdx.x & 31) == 0) { atomicAdd(&stats->subcycles, my_sub); atomicMax(&stats->max_sub, my_max); }
 }
 
+// Radiative-transfer time step (include/arc.h arc_suggest_dt): one streaming pass, 28 B per cell
+// (five fields at the field dtype + Gamma_HI), minimum by warp shuffles and one 64-bit atomicMin per warp on the bits of
+// the (positive) double.  The tau > 0.5 test is products only, in the oracle's order: the same cells qualify.
+template <typename FT>
+__global__ void __launch_bounds__(256) arc_dt_kernel(long long ncell, int scheme, double eps, double sigma1, double d, double Yp,
+                                                    int caseB, int coll, const FT *__restrict__ nHf, const FT *__restrict__ xHIf,
+                                                    const FT *__restrict__ xHeIf, const FT *__restrict__ xHeIIf, const FT *__restrict__ Tf,
+                                                    const double *__restrict__ GammaHI, unsigned long long *out)
+{
+    double best = __longlong_as_double(0x7ff0000000000000ll);
+    unsigned long long used = 0;
+    for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
+        const double nH = (double)nHf[c], x0 = (double)xHIf[c], x1 = (double)xHeIf[c], x2 = (double)xHeIIf[c];
+        const double nHe = nH * Yp / (4.0 * (1.0 - Yp));
+        const double xHII = 1.0 - x0;
+        double xHeIII = 1.0 - x1 - x2; if (xHeIII < 0.0) xHeIII = 0.0;
+        const double ne = nH * xHII + nHe * (x2 + 2.0 * xHeIII);
+        Coef k;
+        rate_table((double)Tf[c], caseB != 0, coll != 0, k);
+        const double C0 = GammaHI[c] + k.cHI * ne, D0 = k.aHII * ne * xHII;
+        const double nHI = __dmul_rn(nH, x0);
+        const double ndot = fabs(nH * (D0 - C0 * x0));
+        if (ndot == 0.0) continue;
+        double dt;
+        if (scheme == ARC_DT_NEUTRAL) {
+            const double tau = __dmul_rn(__dmul_rn(nHI, sigma1), d);
+            if (!(tau > 0.5)) continue;
+            dt = eps * nHI / ndot;
+        } else dt = eps / ((sigma1 * d) * ndot);
+        ++used;
+        best = fmin(best, dt);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));
+        used += __shfl_xor_sync(0xffffffffu, used, o);
+    }
+    if ((threadIdx.x & 31) == 0 && used) {
+        atomicMin(out, (unsigned long long)__double_as_longlong(best));
+        atomicAdd(out + 1, used);
+    }
+}
+
+template <typename FT>
+cudaError_t launch_dt(arc_ctx *c, int scheme, double eps)
+{
+    const long long nb = (c->ncell + 255) / 256;
+    const long long cap = (long long)c->n_sm * 8;
+    FT **f = reinterpret_cast<FT **>(c->f);
+    arc_dt_kernel<FT><<<(int)(nb < cap ? nb : cap), 256, 0, c->stream>>>(c->ncell, scheme, eps, c->spec.sig[0][0], c->dx, c->p.Yp, c->p.caseB,
+                                                                        c->p.coll_ion, f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_dt);
+    return cudaGetLastError();
+}
+
 template <typename FT>
 cudaError_t launch_chem(arc_ctx *c, double dt)
 {
@@ -158,6 +212,11 @@ cudaError_t launch_chem(arc_ctx *c, double dt)
 }
 
 }  // namespace
+
+cudaError_t arc_launch_suggest_dt(arc_ctx *c, int scheme, double eps)
+{
+    return c->dtype == ARC_F32 ? launch_dt<float>(c, scheme, eps) : launch_dt<double>(c, scheme, eps);
+}
 
 cudaError_t arc_launch_chemistry(arc_ctx *c, double dt)
 {

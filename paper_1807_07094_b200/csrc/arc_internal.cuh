@@ -110,6 +110,7 @@ struct arc_ctx {
     SchedState *d_sched = 0;
     DevStats *d_stats = 0;
     double *d_absorbed = 0;           // [ARC_MAX_BINS] reduction scratch
+    unsigned long long *d_dt = 0;     // [2] arc_suggest_dt: min dt (bits of a positive double), cells used
     int n_sm = 0;
     int trace_grid = 0;
     cudaEvent_t ev[8];                // 0..4: trace call (start, after opacity, after kernel, after finalize); 5,6: chemistry
@@ -127,3 +128,4 @@ int arc_trace_occupancy_grid(arc_ctx *c, int nb, int flags);   // flags: 1 log, 
 cudaError_t arc_launch_pix2vec(const int32_t *d_level, const uint32_t *d_pix, int n, double *d_out, cudaStream_t s);
 // arc_chem.cu
 cudaError_t arc_launch_chemistry(arc_ctx *c, double dt);
+cudaError_t arc_launch_suggest_dt(arc_ctx *c, int scheme, double eps);     // result in c->d_dt

@@ -193,6 +193,27 @@ int arc_update_chemistry(arc_ctx *c, double dt_s)
     return ARC_OK;
 }
 
+int arc_suggest_dt(arc_ctx *c, int scheme, double eps, double *dt_s, int64_t *cells_used)
+{
+    if (!c) return ARC_EINVAL;
+    if (!dt_s) return fail(c, ARC_EINVAL, "arc_suggest_dt: dt_s is NULL");
+    if (scheme != ARC_DT_NEUTRAL && scheme != ARC_DT_INTENSITY) return fail(c, ARC_EINVAL, "arc_suggest_dt: scheme must be ARC_DT_NEUTRAL or ARC_DT_INTENSITY");
+    if (!(eps > 0.0) || !std::isfinite(eps)) return fail(c, ARC_EINVAL, "arc_suggest_dt: eps must be finite and > 0");
+    if (!c->have_rates) return fail(c, ARC_ESTATE, "arc_suggest_dt: no valid rates (call arc_trace after setting fields)");
+    if (!c->d_dt) CK(cudaMalloc(&c->d_dt, 2 * sizeof(unsigned long long)));
+    CK(cudaMemsetAsync(c->d_dt, 0xFF, sizeof(unsigned long long), c->stream));        // above the bits of +inf
+    CK(cudaMemsetAsync(c->d_dt + 1, 0, sizeof(unsigned long long), c->stream));
+    CK(arc_launch_suggest_dt(c, scheme, eps));
+    unsigned long long h[2];
+    CK(cudaMemcpyAsync(h, c->d_dt, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    double dt = INFINITY;
+    if (h[0] < 0x7ff0000000000000ull) std::memcpy(&dt, &h[0], sizeof(dt));
+    *dt_s = dt;
+    if (cells_used) *cells_used = (int64_t)h[1];
+    return ARC_OK;
+}
+
 int arc_synchronize(arc_ctx *c)
 {
     if (!c) return ARC_EINVAL;

@@ -70,7 +70,7 @@ def test_enums_match_the_header():
     for name in ("ARC_F32", "ARC_F64", "ARC_HOST", "ARC_DEVICE", "ARC_OK", "ARC_EINVAL", "ARC_ENOMEM", "ARC_ECUDA",
                  "ARC_ESTATE", "ARC_EOVERFLOW", "ARC_END_SPLIT", "ARC_END_DEPLETED", "ARC_END_ESCAPED",
                  "ARC_DEPOSIT_AUTO", "ARC_DEPOSIT_RED", "ARC_DEPOSIT_AGG", "ARC_DEPOSIT_QUAD",
-                 "ARC_GEOM_NONE", "ARC_GEOM_FC", "ARC_GEOM_FC_SECONDARY", "ARC_GEOM_FC2"):
+                 "ARC_GEOM_NONE", "ARC_GEOM_FC", "ARC_GEOM_FC_SECONDARY", "ARC_GEOM_FC2", "ARC_DT_NEUTRAL", "ARC_DT_INTENSITY"):
         m = re.search(rf"\b{name}\s*=\s*(-?\d+)", src)
         assert m, name
         assert int(m.group(1)) == getattr(arc, name), name
