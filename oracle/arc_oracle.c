@@ -218,8 +218,12 @@ static uint64_t ray_key(int32_t src, int32_t level, uint64_t pix)
     return ((uint64_t)(uint32_t)src << 40) | ((uint64_t)level << 32) | pix;
 }
 
-int orc_trace(const orc_params *p, int nb, const double *kappa, int nsrc, const double *pos_cm,
-              const double *Ndot, const double *binfrac, double *A, orc_stats *st, orc_raylog *log)
+/* blocked: NULL, or [nsrc][12 4^l0] bytes, non-zero = that root ray is blocked (anisotropic emission, PAPER.md:88:
+ * "assigning the mean S_nu per ray to a fraction f_esc of the rays, while completely blocking ... the remaining rays").
+ * A blocked root ray does not exist: no packet, no segments, not in emitted. */
+int orc_trace_masked(const orc_params *p, int nb, const double *kappa, int nsrc, const double *pos_cm,
+                     const double *Ndot, const double *binfrac, const uint8_t *blocked, double *A, orc_stats *st,
+                     orc_raylog *log)
 {
     const int N = p->N;
     const double dx = p->box_cm / (double)N;
@@ -235,10 +239,13 @@ int orc_trace(const orc_params *p, int nb, const double *kappa, int nsrc, const 
     for (int s = 0; s < nsrc; ++s) {
         double g[3];
         for (int a = 0; a < 3; ++a) g[a] = pos_cm[3 * s + a] / dx;      /* grid units */
-        for (int v = 0; v < nb; ++v) st->emitted[v] += Ndot[s] * binfrac[s * nb + v];
         /* root rays: all pixels of level l0, r = 0, tau = 0 */
         const uint64_t npix0 = 12ull << (2 * p->l0);
+        uint64_t nopen = npix0;
+        if (blocked) for (uint64_t k = 0; k < npix0; ++k) if (blocked[(uint64_t)s * npix0 + k]) --nopen;
+        for (int v = 0; v < nb; ++v) st->emitted[v] += (Ndot[s] * binfrac[s * nb + v]) / (double)npix0 * (double)nopen;
         for (uint64_t k = npix0; k-- > 0;) {
+            if (blocked && blocked[(uint64_t)s * npix0 + k]) continue;
             if (top == cap) { cap *= 2; stack = (ray_rec *)realloc(stack, cap * sizeof(ray_rec)); if (!stack) return -2; }
             ray_rec *r = &stack[top++];
             r->src = s; r->level = p->l0; r->pix = k; r->r0 = 0.0;
@@ -375,6 +382,12 @@ int orc_trace(const orc_params *p, int nb, const double *kappa, int nsrc, const 
     }
     free(stack);
     return 0;
+}
+
+int orc_trace(const orc_params *p, int nb, const double *kappa, int nsrc, const double *pos_cm,
+              const double *Ndot, const double *binfrac, double *A, orc_stats *st, orc_raylog *log)
+{
+    return orc_trace_masked(p, nb, kappa, nsrc, pos_cm, Ndot, binfrac, NULL, A, st, log);
 }
 
 /* ------------------------------------------------------------------------------------------

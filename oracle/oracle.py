@@ -130,8 +130,9 @@ def opacity(w, fields=None, **override) -> np.ndarray:
 
 
 def trace(w, kappa=None, fields=None, log=False, cap_rays=2_000_000, cap_cells=60_000_000,
-          sources=None, **override):
-    """-> (A[cell, v] absorbed photons/s, stats dict, raylog dict or None)."""
+          sources=None, blocked=None, **override):
+    """-> (A[cell, v] absorbed photons/s, stats dict, raylog dict or None).
+    blocked: None or uint8 [nsrc, 12 4^l0], non-zero = root ray blocked (anisotropic emission)."""
     p = make_params(w, **override)
     if kappa is None:
         kappa = opacity(w, fields, **override)
@@ -153,8 +154,15 @@ def trace(w, kappa=None, fields=None, log=False, cap_rays=2_000_000, cap_cells=6
         for k, v in arrs.items():
             setattr(rl, k, v.ctypes.data)
         keep = arrs
-    rc = lib().orc_trace(C.byref(p), w.nb, _p(kappa), len(Nd), _p(pos), _p(Nd), _p(bf), _p(A),
-                         C.byref(st), C.byref(rl) if rl is not None else None)
+    bl = None
+    if blocked is not None:
+        bl = np.ascontiguousarray(blocked, dtype=np.uint8)
+        if sources is not None:
+            bl = np.ascontiguousarray(bl[sources])
+        assert bl.shape == (len(Nd), 12 << (2 * p.l0))
+    rc = lib().orc_trace_masked(C.byref(p), w.nb, _p(kappa), len(Nd), _p(pos), _p(Nd), _p(bf),
+                                _p(bl) if bl is not None else None, _p(A),
+                                C.byref(st), C.byref(rl) if rl is not None else None)
     if rc != 0:
         raise RuntimeError(f"orc_trace failed: {rc}")
     nb = w.nb
