@@ -160,6 +160,13 @@ int arc_get_accum(arc_ctx *c, double *A, int where);
  * trace has been done since the fields were last set. */
 int arc_update_chemistry(arc_ctx *c, double dt_s);
 
+/* Anisotropic emission: blocked[s * npix0 + p] != 0 blocks root ray p (nested pixel of level l0,
+ * npix0 = 12 * 4^l0) of source s: it does not exist - no packet, no segments, not in `emitted`; the open rays carry the
+ * mean rate per ray Ndot f_nu / npix0, so a source with a fraction f_esc of its rays open emits f_esc Ndot.
+ * `level` must equal arc_params.l0 at the time of the call and of every later arc_trace (ARC_ESTATE otherwise).
+ * blocked: HOST pointer, nsrc * npix0 bytes, copied; NULL clears the mask.  arc_set_sources clears it too. */
+int arc_set_emission_mask(arc_ctx *c, const uint8_t *blocked, int level);
+
 /* Radiative-transfer time step, from the CURRENT fields and the rates of the last arc_trace:
  * per cell dn_HI/dt = n_H (alpha_HII n_e x_HII - (Gamma_HI + C_HI n_e) x_HI) (Eq. 4);
  *   scheme ARC_DT_NEUTRAL   (i):  min over cells with tau = n_HI sigma_1 d > 0.5 of eps n_HI / |dn_HI/dt|   (:182-190)

@@ -28,7 +28,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libarc_b200.so")
 
 EXPORTS = ["arc_create_grid", "arc_destroy", "arc_default_params", "arc_set_params", "arc_set_stream",
-           "arc_set_fields", "arc_get_fields", "arc_set_spectrum", "arc_set_sources", "arc_trace",
+           "arc_set_fields", "arc_get_fields", "arc_set_spectrum", "arc_set_sources", "arc_set_emission_mask", "arc_trace",
            "arc_get_rates", "arc_get_accum", "arc_update_chemistry", "arc_suggest_dt", "arc_synchronize", "arc_get_stats",
            "arc_trace_debug", "arc_pix2vec", "arc_last_error", "arc_version"]
 
@@ -95,6 +95,7 @@ def lib():
         l.arc_get_accum.argtypes = [vp, vp, i32]
         l.arc_update_chemistry.argtypes = [vp, dbl]
         l.arc_suggest_dt.argtypes = [vp, i32, dbl, vp, vp]
+        l.arc_set_emission_mask.argtypes = [vp, vp, i32]
         l.arc_synchronize.argtypes = [vp]
         l.arc_get_stats.argtypes = [vp, C.POINTER(arc_stats)]
         l.arc_trace_debug.argtypes = [vp, i32, C.POINTER(arc_raylog)]
@@ -223,6 +224,14 @@ def arc_update_chemistry(ctx, dt_s: float):
 ARC_DT_NEUTRAL, ARC_DT_INTENSITY = 1, 2
 
 
+def arc_set_emission_mask(ctx, blocked, level: int):
+    """blocked: None (clear) or uint8 [nsrc, 12 4^level], non-zero = root ray blocked."""
+    if blocked is None:
+        return _check(ctx, lib().arc_set_emission_mask(ctx, None, int(level)))
+    b = np.ascontiguousarray(blocked, dtype=np.uint8)
+    return _check(ctx, lib().arc_set_emission_mask(ctx, b.ctypes.data_as(C.c_void_p), int(level)))
+
+
 def arc_suggest_dt(ctx, scheme: int = ARC_DT_NEUTRAL, eps: float = 0.1):
     """-> (dt_s, cells that entered the minimum)."""
     dt = C.c_double(0.0)
@@ -339,6 +348,9 @@ class Context:
         A = np.zeros((self.w.ncell, self.nb))
         arc_get_accum(self.ctx, A)
         return A
+
+    def set_emission_mask(self, blocked, level=None):
+        return arc_set_emission_mask(self.ctx, blocked, int(self.w.params["l0"]) if level is None else int(level))
 
     def suggest_dt(self, scheme=ARC_DT_NEUTRAL, eps=0.1):
         return arc_suggest_dt(self.ctx, scheme, eps)

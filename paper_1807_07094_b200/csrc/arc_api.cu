@@ -91,7 +91,7 @@ int arc_destroy(arc_ctx *c)
     if (!c) return ARC_OK;
     cudaStreamSynchronize(c->stream);
     for (int i = 0; i < 5; ++i) cudaFree(c->f[i]);
-    cudaFree(c->d_rates); cudaFree(c->d_sched); cudaFree(c->d_stats); cudaFree(c->d_absorbed); cudaFree(c->d_dt);
+    cudaFree(c->d_rates); cudaFree(c->d_sched); cudaFree(c->d_stats); cudaFree(c->d_absorbed); cudaFree(c->d_dt); cudaFree(c->d_blocked);
     cudaFree(c->d_kappa); cudaFree(c->d_A); cudaFree(c->d_src_g); cudaFree(c->d_src_S);
     cudaFree(c->d_stacks); cudaFree(c->d_queue); cudaFree(c->d_qseq);
     for (int i = 0; i < 8; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
@@ -208,6 +208,8 @@ int arc_set_sources(arc_ctx *c, int nsrc, const double *pos_cm, const double *Nd
     }
     CK(cudaStreamSynchronize(c->stream));
     cudaFree(c->d_src_g); cudaFree(c->d_src_S); c->d_src_g = nullptr; c->d_src_S = nullptr;
+    cudaFree(c->d_blocked); c->d_blocked = nullptr; c->mask_level = -1;
+    c->h_src_S = S;
     if (nsrc > 0) {
         CK(cudaMalloc(&c->d_src_g, g.size() * sizeof(double)));
         CK(cudaMalloc(&c->d_src_S, S.size() * sizeof(double)));
@@ -216,6 +218,35 @@ int arc_set_sources(arc_ctx *c, int nsrc, const double *pos_cm, const double *Nd
     }
     c->nsrc = nsrc;
     c->have_src = true;
+    c->have_rates = false;
+    return ARC_OK;
+}
+
+int arc_set_emission_mask(arc_ctx *c, const uint8_t *blocked, int level)
+{
+    if (!c) return ARC_EINVAL;
+    if (!c->have_src) return fail(c, ARC_ESTATE, "arc_set_emission_mask: call arc_set_sources first");
+    const int nb = c->spec.nb;
+    CK(cudaStreamSynchronize(c->stream));
+    cudaFree(c->d_blocked); c->d_blocked = nullptr; c->mask_level = -1;
+    for (int v = 0; v < ARC_MAX_BINS; ++v) c->emitted[v] = 0.0;
+    if (!blocked) {
+        for (int s = 0; s < c->nsrc; ++s) for (int v = 0; v < nb; ++v) c->emitted[v] += c->h_src_S[(size_t)s * nb + v];
+        c->have_rates = false;
+        return ARC_OK;
+    }
+    if (level != c->p.l0) return fail(c, ARC_EINVAL, "arc_set_emission_mask: level must equal arc_params.l0");
+    const size_t npix0 = (size_t)12 << (2 * level);
+    for (int s = 0; s < c->nsrc; ++s) {
+        size_t nopen = npix0;
+        for (size_t p = 0; p < npix0; ++p) if (blocked[(size_t)s * npix0 + p]) --nopen;
+        for (int v = 0; v < nb; ++v) c->emitted[v] += c->h_src_S[(size_t)s * nb + v] / (double)npix0 * (double)nopen;
+    }
+    if (c->nsrc > 0) {
+        CK(cudaMalloc(&c->d_blocked, (size_t)c->nsrc * npix0));
+        CK(cudaMemcpy(c->d_blocked, blocked, (size_t)c->nsrc * npix0, cudaMemcpyHostToDevice));
+    }
+    c->mask_level = level;
     c->have_rates = false;
     return ARC_OK;
 }

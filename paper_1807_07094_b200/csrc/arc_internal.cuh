@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string>
+#include <vector>
 #include "../../include/arc.h"
 
 #define ARC_WARPS_PER_BLOCK 8
@@ -71,6 +72,7 @@ struct TraceArgs {
     double *A;                 // [cell][nbp] absorbed photons/s (entries nb..nbp-1 stay zero)
     const double *src_g;       // [nsrc][3] source position in grid units
     const double *src_S;       // [nsrc][nb] Ndot * binfrac
+    const unsigned char *blocked;   // NULL or [nsrc][12 4^l0]: blocked root rays (anisotropic emission)
     unsigned char *stacks;     // n_warps * ARC_STACK_CAP family records
     unsigned char *queue;      // ARC_QUEUE_CAP family records
     unsigned long long *qseq;  // ARC_QUEUE_CAP slot sequence numbers
@@ -101,6 +103,8 @@ struct arc_ctx {
     bool have_fields = false, have_spec = false, have_src = false, have_rates = false;
     int nsrc = 0;
     double *d_src_g = 0, *d_src_S = 0;
+    std::vector<double> h_src_S;      // host copy of Ndot * binfrac (emitted with an emission mask)
+    unsigned char *d_blocked = 0; int mask_level = -1;     // arc_set_emission_mask
     double emitted[ARC_MAX_BINS];
     void *d_kappa = 0; int kappa_nb = 0;
     double *d_A = 0; int A_nb = 0;

@@ -41,6 +41,7 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
     if (!c->have_fields) return fail(c, ARC_ESTATE, "arc_trace: no fields set (arc_set_fields)");
     if (!c->have_spec) return fail(c, ARC_ESTATE, "arc_trace: no spectrum set (arc_set_spectrum)");
     if (!c->have_src) return fail(c, ARC_ESTATE, "arc_trace: no sources set (arc_set_sources)");
+    if (c->d_blocked && c->mask_level != c->p.l0) return fail(c, ARC_ESTATE, "arc_trace: the emission mask was set for another l0 (arc_set_emission_mask)");
     const int nb = c->spec.nb;
     // persistent grid: what is co-resident (SM count x blocks per SM), or the caller's override
     const int flags = (log ? 3 : (c->p.digest ? 2 : 0)) | (c->p.geom_corr ? 4 : 0);     // FLAG_LOG 1, FLAG_DIGEST 2, FLAG_GEOM 4
@@ -74,7 +75,7 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
     a.tau_term = c->p.tau_term;
     a.cpix = std::sqrt(3.14159265358979323846 / 3.0);                     // sqrt(Omega_l) = cpix 2^-l (G26)
     a.geom = c->p.geom_corr;
-    a.kappa = c->d_kappa; a.A = c->d_A; a.src_g = c->d_src_g; a.src_S = c->d_src_S;
+    a.kappa = c->d_kappa; a.A = c->d_A; a.src_g = c->d_src_g; a.src_S = c->d_src_S; a.blocked = c->d_blocked;
     a.stacks = c->d_stacks; a.queue = c->d_queue; a.qseq = c->d_qseq; a.sched = c->d_sched; a.stats = c->d_stats;
     a.fam_per_src = 3u << (2 * c->p.l0);
     a.seed_total = (unsigned long long)c->nsrc * a.fam_per_src;

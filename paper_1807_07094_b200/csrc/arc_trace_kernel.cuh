@@ -342,6 +342,13 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
         int cell = 0;                          // N <= 1024: N^3 <= 2^30
         int end = -1;
         unsigned long long h = 0; unsigned int seq = 0;
+        if (active && a.blocked != nullptr) {                 // anisotropic emission: a blocked root ray does not exist
+            const Rec *rp = &STK(top + myfam);
+            if ((int)rp->level == a.l0) {
+                const size_t ip = (size_t)rp->src * ((size_t)12 << (2 * a.l0)) + (4u * rp->fam + (uint32_t)(lane & 3));
+                if (a.blocked[ip]) active = false;
+            }
+        }
         if (active) {
             const Rec *rp = &STK(top + myfam);
             src = rp->src; level = (int)rp->level; pix = 4u * rp->fam + (uint32_t)(lane & 3);

@@ -27,9 +27,11 @@ def assert_close(a, b, rtol, what, atol_frac=1e-12):
 
 def gpu_raylog_to_dict(key, seq, cell):
     """(key, seq, cell) entries -> {(src, level, pix): (tuple(cells), end)}"""
+    out = {}
+    if len(key) == 0:                      # (every root ray blocked: no ray at all)
+        return out
     order = np.lexsort((seq, key))
     key, seq, cell = key[order], seq[order], cell[order]
-    out = {}
     bounds = np.flatnonzero(np.diff(key)) + 1
     starts = np.concatenate([[0], bounds]); stops = np.concatenate([bounds, [len(key)]])
     for a, b in zip(starts, stops):
