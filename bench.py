@@ -61,14 +61,19 @@ def hbm_peak():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(config: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one tracer launch on this workload, from the committed
-    `ncu --set full` capture (profiles/ncu_traffic.json names the capture); None if this workload has none."""
+def ncu_capture(config: str) -> dict:
+    """What the committed `ncu --set full` capture of the tracer on this workload measured (profiles/ncu_traffic.json
+    names the capture): DRAM bytes and warp instructions per launch.  {} if this workload has none."""
     try:
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-            return json.load(f).get(config, {}).get("dram_bytes_per_launch")
+            return json.load(f).get(config, {})
     except OSError:
-        return None
+        return {}
+
+
+def ncu_traffic(config: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one tracer launch on this workload, or None."""
+    return ncu_capture(config).get("dram_bytes_per_launch")
 
 
 def algorithmic_bytes_per_segment(w) -> int:
@@ -319,6 +324,16 @@ def run_cuda(args):
             "segments_per_deposit_record": seg_per_record,
             "host_wall_s": wall,
         }
+        cap = ncu_capture(args.config)
+        if cap.get("warp_instructions_per_segment") and clocks and clocks.get("sm_mhz") and kms > 0:
+            # the limit that binds: issue slots.  4 schedulers x SMs x SM clock under load
+            import torch as _t
+            n_sm = _t.cuda.get_device_properties(local).multi_processor_count
+            ach = cap["warp_instructions_per_segment"] * tot_seg / (kms * 1e-3) / 1e9
+            pk = 4 * n_sm * clocks["sm_mhz"] * 1e6 / 1e9
+            line["issue"] = {"bound": "issue", "achieved": ach, "peak": pk, "unit": "G warp-instructions/s", "frac": ach / pk,
+                             "warp_instructions_per_segment": cap["warp_instructions_per_segment"],
+                             "peak_source": f"4 schedulers x {n_sm} SMs x {clocks['sm_mhz']:.0f} MHz (SM clock sampled under load)"}
         if world == 1 and not args.no_cpu_baseline:
             seg, secs, S, cores = oracle_sample(w, budget_s=12.0)
             line["cpu_baseline"] = {"value": seg / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
