@@ -53,6 +53,8 @@ typedef struct {
     double x_floor;
     int32_t geom_corr;        /* 0 none, 1 f_c (Eq. 2), 2 f_c + secondary f'_c (Eq. 3), 3 f_c squared */
     int32_t pad_;
+    double thin_tau;          /* optical depth (softest bin) below which a source's surroundings count as
+                                 optically thin, 0.1 in the paper; 0 = the approximation is off */
 } orc_params;
 
 typedef struct {
@@ -221,9 +223,17 @@ static uint64_t ray_key(int32_t src, int32_t level, uint64_t pix)
 /* blocked: NULL, or [nsrc][12 4^l0] bytes, non-zero = that root ray is blocked (anisotropic emission, PAPER.md:88:
  * "assigning the mean S_nu per ray to a fraction f_esc of the rays, while completely blocking ... the remaining rays").
  * A blocked root ray does not exist: no packet, no segments, not in emitted. */
-int orc_trace_masked(const orc_params *p, int nb, const double *kappa, int nsrc, const double *pos_cm,
-                     const double *Ndot, const double *binfrac, const uint8_t *blocked, double *A, orc_stats *st,
-                     orc_raylog *log)
+/* Optically thin inner region (readings G33-G37), active when p->thin_tau > 0:
+ *  Rstart[s] (grid units; NULL = all 0): radius found by the PREVIOUS trace.  Where it is > 0, (iii) every cell whose
+ *  centre lies within Rstart of the source receives S_nu kappa_nu V / (4 pi r^2) absorbed photons/s (Eq. 1 for small
+ *  tau, dilution 4 pi r^2; r^2 not below (d/2)^2), and (iv) the rays start at r = Rstart with tau = 0, at the level
+ *  they would have there (r_split(l-1) <= Rstart < r_split(l)).
+ *  Rnext[s] (may be NULL): (ii) the minimum over this trace's rays of the radius up to which tau (softest bin) stays
+ *  below thin_tau: the START radius of the segment in which tau reaches thin_tau, or the radius at which a ray ends
+ *  (leaves the box / is depleted) with tau still below it; 0 if the source traced no ray. */
+int orc_trace_thin(const orc_params *p, int nb, const double *kappa, int nsrc, const double *pos_cm,
+                   const double *Ndot, const double *binfrac, const uint8_t *blocked, const double *Rstart,
+                   double *Rnext, double *A, orc_stats *st, orc_raylog *log)
 {
     const int N = p->N;
     const double dx = p->box_cm / (double)N;
@@ -244,11 +254,34 @@ int orc_trace_masked(const orc_params *p, int nb, const double *kappa, int nsrc,
         uint64_t nopen = npix0;
         if (blocked) for (uint64_t k = 0; k < npix0; ++k) if (blocked[(uint64_t)s * npix0 + k]) --nopen;
         for (int v = 0; v < nb; ++v) st->emitted[v] += (Ndot[s] * binfrac[s * nb + v]) / (double)npix0 * (double)nopen;
-        for (uint64_t k = npix0; k-- > 0;) {
-            if (blocked && blocked[(uint64_t)s * npix0 + k]) continue;
+        const int thin = p->thin_tau > 0.0;
+        const double R0 = (thin && Rstart) ? Rstart[s] : 0.0;
+        double Rmin = INFINITY;
+        int lroot = p->l0;
+        if (R0 > 0.0) {
+            /* (iv) the level rays have at radius R0 */
+            while (lroot < p->Lmax && orc_rsplit(p->Phi, lroot, p->Lmax) <= R0) ++lroot;
+            /* (iii) cells whose centre is within R0: thin-limit absorption, no rays */
+            const double R2 = R0 * R0;
+            for (int iz = 0; iz < N; ++iz) for (int iy = 0; iy < N; ++iy) for (int ix = 0; ix < N; ++ix) {
+                const double ex = ((double)ix + 0.5) - g[0], ey = ((double)iy + 0.5) - g[1], ez = ((double)iz + 0.5) - g[2];
+                const double d2 = (ex * ex + ey * ey) + ez * ez;
+                if (!(d2 <= R2)) continue;
+                const double r2 = d2 < 0.25 ? 0.25 : d2;
+                const int64_t c = ((int64_t)iz * N + iy) * N + ix;
+                for (int v = 0; v < nb; ++v) {
+                    const double a_v = (Ndot[s] * binfrac[s * nb + v]) / (double)npix0 * (double)nopen
+                                       * (kappa[c * nb + v] * dx) / (4.0 * ORC_PI * r2);
+                    A[c * nb + v] += a_v; st->absorbed[v] += a_v;
+                }
+            }
+        }
+        const uint64_t npixr = 12ull << (2 * lroot);
+        for (uint64_t k = npixr; k-- > 0;) {
+            if (blocked && blocked[(uint64_t)s * npix0 + (k >> (2 * (lroot - p->l0)))]) continue;   /* blocked level-l0 ancestor */
             if (top == cap) { cap *= 2; stack = (ray_rec *)realloc(stack, cap * sizeof(ray_rec)); if (!stack) return -2; }
             ray_rec *r = &stack[top++];
-            r->src = s; r->level = p->l0; r->pix = k; r->r0 = 0.0;
+            r->src = s; r->level = lroot; r->pix = k; r->r0 = R0;
             for (int v = 0; v < nb; ++v) r->tau[v] = 0.0;
         }
         while (top > 0) {
@@ -336,6 +369,7 @@ int orc_trace_masked(const orc_params *p, int nb, const double *kappa, int nsrc,
                                 A[(cn >= 0 ? cn : c) * nb + v] += off; st->absorbed[v] += off;
                             }
                         }
+                        if (v == 0 && thin && tau[0] < p->thin_tau && tau[0] + dtau >= p->thin_tau && r < Rmin) Rmin = r;   /* (ii) */
                         tau[v] = tau[v] + dtau;
                     }
                     st->segments++;
@@ -374,14 +408,23 @@ int orc_trace_masked(const orc_params *p, int nb, const double *kappa, int nsrc,
                     }
                 }
             }
+            if (thin && end != ORC_END_SPLIT && tau[0] < p->thin_tau && r < Rmin) Rmin = r;      /* (ii): ended still thin */
             st->ends[end]++;
             h = mix64(h ^ (0xE0ull + (uint64_t)end));
             st->digest += h;
             if (log) { log->end[lr] = end; log->r_end[lr] = r; }
         }
+        if (Rnext) Rnext[s] = (thin && Rmin < INFINITY) ? Rmin : 0.0;
     }
     free(stack);
     return 0;
+}
+
+int orc_trace_masked(const orc_params *p, int nb, const double *kappa, int nsrc, const double *pos_cm,
+                     const double *Ndot, const double *binfrac, const uint8_t *blocked, double *A, orc_stats *st,
+                     orc_raylog *log)
+{
+    return orc_trace_thin(p, nb, kappa, nsrc, pos_cm, Ndot, binfrac, blocked, NULL, NULL, A, st, log);
 }
 
 int orc_trace(const orc_params *p, int nb, const double *kappa, int nsrc, const double *pos_cm,

@@ -32,7 +32,7 @@ class Params(C.Structure):
                 ("l0", C.c_int32), ("Lmax", C.c_int32), ("Phi", C.c_double), ("tau_term", C.c_double),
                 ("Yp", C.c_double), ("isothermal", C.c_int32), ("caseB", C.c_int32),
                 ("coll_ion", C.c_int32), ("max_subcycles", C.c_int32), ("eps_sub", C.c_double),
-                ("x_floor", C.c_double), ("geom_corr", C.c_int32), ("pad_", C.c_int32)]
+                ("x_floor", C.c_double), ("geom_corr", C.c_int32), ("pad_", C.c_int32), ("thin_tau", C.c_double)]
 
 
 class Stats(C.Structure):
@@ -84,7 +84,7 @@ def make_params(w, **override) -> Params:
                   Lmax=int(d["Lmax"]), Phi=float(d["Phi"]), tau_term=float(d["tau_term"]),
                   Yp=float(d["Yp"]), isothermal=int(d["isothermal"]), caseB=int(d["caseB"]),
                   coll_ion=int(d["coll_ion"]), max_subcycles=int(d["max_subcycles"]),
-                  eps_sub=float(d["eps_sub"]), x_floor=float(d["x_floor"]), geom_corr=int(d.get("geom_corr", 0)))
+                  eps_sub=float(d["eps_sub"]), x_floor=float(d["x_floor"]), geom_corr=int(d.get("geom_corr", 0)), thin_tau=float(d.get("thin_tau", 0.0)))
 
 
 # ---- O1/O2 -------------------------------------------------------------------------------
@@ -130,9 +130,11 @@ def opacity(w, fields=None, **override) -> np.ndarray:
 
 
 def trace(w, kappa=None, fields=None, log=False, cap_rays=2_000_000, cap_cells=60_000_000,
-          sources=None, blocked=None, **override):
+          sources=None, blocked=None, Rstart=None, **override):
     """-> (A[cell, v] absorbed photons/s, stats dict, raylog dict or None).
-    blocked: None or uint8 [nsrc, 12 4^l0], non-zero = root ray blocked (anisotropic emission)."""
+    blocked: None or uint8 [nsrc, 12 4^l0], non-zero = root ray blocked (anisotropic emission).
+    With thin_tau > 0 (optically thin inner region): Rstart = per-source radii [cells] found by the
+    previous trace (None = 0), and stats["R_thin"] = the radii this trace found."""
     p = make_params(w, **override)
     if kappa is None:
         kappa = opacity(w, fields, **override)
@@ -160,9 +162,16 @@ def trace(w, kappa=None, fields=None, log=False, cap_rays=2_000_000, cap_cells=6
         if sources is not None:
             bl = np.ascontiguousarray(bl[sources])
         assert bl.shape == (len(Nd), 12 << (2 * p.l0))
-    rc = lib().orc_trace_masked(C.byref(p), w.nb, _p(kappa), len(Nd), _p(pos), _p(Nd), _p(bf),
-                                _p(bl) if bl is not None else None, _p(A),
-                                C.byref(st), C.byref(rl) if rl is not None else None)
+    Rs = None
+    if Rstart is not None:
+        Rs = _f64(np.asarray(Rstart, dtype=np.float64))
+        if sources is not None and len(Rs) != len(Nd):
+            Rs = _f64(Rs[sources])
+        assert Rs.shape == (len(Nd),)
+    Rn = np.zeros(len(Nd))
+    rc = lib().orc_trace_thin(C.byref(p), w.nb, _p(kappa), len(Nd), _p(pos), _p(Nd), _p(bf),
+                              _p(bl) if bl is not None else None, _p(Rs) if Rs is not None else None, _p(Rn), _p(A),
+                              C.byref(st), C.byref(rl) if rl is not None else None)
     if rc != 0:
         raise RuntimeError(f"orc_trace failed: {rc}")
     nb = w.nb
@@ -170,7 +179,7 @@ def trace(w, kappa=None, fields=None, log=False, cap_rays=2_000_000, cap_cells=6
                  max_stack=int(st.max_stack), splits=np.array(st.splits[:], dtype=np.uint64),
                  rays_level=np.array(st.rays_level[:], dtype=np.uint64), ends=np.array(st.ends[:], dtype=np.uint64),
                  emitted=np.array(st.emitted[:nb]), absorbed=np.array(st.absorbed[:nb]),
-                 escaped=np.array(st.escaped[:nb]))
+                 escaped=np.array(st.escaped[:nb]), R_thin=Rn)
     raylog = None
     if log:
         nr, ncs = int(rl.n_rays), int(rl.n_cells)
