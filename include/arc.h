@@ -71,6 +71,12 @@ typedef struct arc_params {
     int32_t deposit;        /* how segments reach the accumulators: ARC_DEPOSIT_AUTO | _RED | _AGG | _QUAD        */
     int32_t geom_corr;      /* ARC_GEOM_NONE | _FC | _FC_SECONDARY | _FC2; needs deposit = AUTO */
     int32_t reserved0;      /* keep 0                                                                 */
+    double  thin_tau;       /* optically thin inner region: 0 = off; > 0 (0.1 in the paper): every
+                               arc_trace records, per source, the radius up to which tau of the first (softest) bin stays
+                               below thin_tau on every ray, and the NEXT arc_trace gives the cells within that radius the
+                               thin-limit absorption S kappa V / (4 pi r^2) and starts the rays there (tau = 0, at the
+                               level they have at that radius).  Needs deposit = AUTO and geom_corr = NONE; arc_trace
+                               then synchronises.  Radii: arc_get_thin_radii / arc_set_thin_radii.                */
 } arc_params;
 
 /* Per-cell outputs of arc_trace (PAPER.md:83 Eq. 1, :134-138, :170): DEVICE pointers, N^3 doubles each. */
@@ -166,6 +172,12 @@ int arc_update_chemistry(arc_ctx *c, double dt_s);
  * `level` must equal arc_params.l0 at the time of the call and of every later arc_trace (ARC_ESTATE otherwise).
  * blocked: HOST pointer, nsrc * npix0 bytes, copied; NULL clears the mask.  arc_set_sources clears it too. */
 int arc_set_emission_mask(arc_ctx *c, const uint8_t *blocked, int level);
+
+/* Optically thin inner region (arc_params.thin_tau > 0): the per-source radii, in CELLS, that the next arc_trace will use
+ * (found by the last one; 0 after arc_set_sources).  HOST pointers, nsrc doubles.  arc_set_thin_radii: values must be
+ * finite and >= 0 (0 = that source traces from r = 0). */
+int arc_get_thin_radii(arc_ctx *c, double *R_cells);
+int arc_set_thin_radii(arc_ctx *c, const double *R_cells);
 
 /* Radiative-transfer time step, from the CURRENT fields and the rates of the last arc_trace:
  * per cell dn_HI/dt = n_H (alpha_HII n_e x_HII - (Gamma_HI + C_HI n_e) x_HI) (Eq. 4);

@@ -28,7 +28,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libarc_b200.so")
 
 EXPORTS = ["arc_create_grid", "arc_destroy", "arc_default_params", "arc_set_params", "arc_set_stream",
-           "arc_set_fields", "arc_get_fields", "arc_set_spectrum", "arc_set_sources", "arc_set_emission_mask", "arc_trace",
+           "arc_set_fields", "arc_get_fields", "arc_set_spectrum", "arc_set_sources", "arc_set_emission_mask", "arc_get_thin_radii", "arc_set_thin_radii", "arc_trace",
            "arc_get_rates", "arc_get_accum", "arc_update_chemistry", "arc_suggest_dt", "arc_synchronize", "arc_get_stats",
            "arc_trace_debug", "arc_pix2vec", "arc_last_error", "arc_version"]
 
@@ -44,7 +44,7 @@ class arc_params(C.Structure):
                 ("Yp", C.c_double), ("isothermal", C.c_int32), ("caseB", C.c_int32), ("coll_ion", C.c_int32),
                 ("max_subcycles", C.c_int32), ("eps_sub", C.c_double), ("x_floor", C.c_double),
                 ("digest", C.c_int32), ("async_", C.c_int32), ("trace_blocks", C.c_int32), ("deposit", C.c_int32),
-                ("geom_corr", C.c_int32), ("reserved0", C.c_int32)]
+                ("geom_corr", C.c_int32), ("reserved0", C.c_int32), ("thin_tau", C.c_double)]
 
 
 class arc_rates(C.Structure):
@@ -96,6 +96,8 @@ def lib():
         l.arc_update_chemistry.argtypes = [vp, dbl]
         l.arc_suggest_dt.argtypes = [vp, i32, dbl, vp, vp]
         l.arc_set_emission_mask.argtypes = [vp, vp, i32]
+        l.arc_get_thin_radii.argtypes = [vp, vp]
+        l.arc_set_thin_radii.argtypes = [vp, vp]
         l.arc_synchronize.argtypes = [vp]
         l.arc_get_stats.argtypes = [vp, C.POINTER(arc_stats)]
         l.arc_trace_debug.argtypes = [vp, i32, C.POINTER(arc_raylog)]
@@ -224,6 +226,18 @@ def arc_update_chemistry(ctx, dt_s: float):
 ARC_DT_NEUTRAL, ARC_DT_INTENSITY = 1, 2
 
 
+def arc_get_thin_radii(ctx, nsrc: int) -> np.ndarray:
+    """radii [cells] the next arc_trace will use (optically thin inner region)."""
+    R = np.zeros(int(nsrc))
+    _check(ctx, lib().arc_get_thin_radii(ctx, R.ctypes.data_as(C.c_void_p)))
+    return R
+
+
+def arc_set_thin_radii(ctx, R):
+    R = np.ascontiguousarray(R, dtype=np.float64)
+    return _check(ctx, lib().arc_set_thin_radii(ctx, R.ctypes.data_as(C.c_void_p)))
+
+
 def arc_set_emission_mask(ctx, blocked, level: int):
     """blocked: None (clear) or uint8 [nsrc, 12 4^level], non-zero = root ray blocked."""
     if blocked is None:
@@ -311,6 +325,7 @@ class Context:
                 arc_set_stream(self.ctx, stream)
             arc_set_spectrum(self.ctx, w.E_eV, w.sig_HI, w.sig_HeI, w.sig_HeII)
             arc_set_sources(self.ctx, w.src_pos_cm, w.src_Ndot, w.src_binfrac)
+            self._nsrc = w.nsrc
             self.set_fields(fields if fields is not None else w.fields())
         except Exception:
             self.close()
@@ -327,6 +342,7 @@ class Context:
 
     def set_sources(self, idx):
         w = self.w
+        self._nsrc = len(idx)
         arc_set_sources(self.ctx, w.src_pos_cm[idx], w.src_Ndot[idx], w.src_binfrac[idx])
 
     def get_fields(self):
@@ -348,6 +364,15 @@ class Context:
         A = np.zeros((self.w.ncell, self.nb))
         arc_get_accum(self.ctx, A)
         return A
+
+    def thin_radii(self):
+        """radii [cells] the next trace will use (optically thin inner region)"""
+        return arc_get_thin_radii(self.ctx, self._nsrc)
+
+    def set_thin_radii(self, R):
+        R = np.ascontiguousarray(R, dtype=np.float64)
+        assert R.shape == (self._nsrc,)
+        return arc_set_thin_radii(self.ctx, R)
 
     def set_emission_mask(self, blocked, level=None):
         return arc_set_emission_mask(self.ctx, blocked, int(self.w.params["l0"]) if level is None else int(level))

@@ -37,7 +37,7 @@ void arc_default_params(arc_params *p)
     std::memset(p, 0, sizeof(*p));
     p->l0 = 1; p->Lmax = 13; p->Phi = 3.0; p->tau_term = 30.0; p->Yp = 0.0;
     p->isothermal = 1; p->caseB = 1; p->coll_ion = 0; p->max_subcycles = 4096;
-    p->eps_sub = 0.1; p->x_floor = 1e-12; p->digest = 0; p->async = 0; p->trace_blocks = 0; p->deposit = ARC_DEPOSIT_AUTO; p->geom_corr = ARC_GEOM_NONE; p->reserved0 = 0;
+    p->eps_sub = 0.1; p->x_floor = 1e-12; p->digest = 0; p->async = 0; p->trace_blocks = 0; p->deposit = ARC_DEPOSIT_AUTO; p->geom_corr = ARC_GEOM_NONE; p->reserved0 = 0; p->thin_tau = 0.0;
 }
 
 int arc_create_grid(arc_ctx **out, int N, double box_cm, int dtype)
@@ -92,6 +92,7 @@ int arc_destroy(arc_ctx *c)
     cudaStreamSynchronize(c->stream);
     for (int i = 0; i < 5; ++i) cudaFree(c->f[i]);
     cudaFree(c->d_rates); cudaFree(c->d_sched); cudaFree(c->d_stats); cudaFree(c->d_absorbed); cudaFree(c->d_dt); cudaFree(c->d_blocked);
+    cudaFree(c->d_Rstart); cudaFree(c->d_Rnext); cudaFree(c->d_seed_prefix); cudaFree(c->d_src_level); cudaFree(c->d_Sopen);
     cudaFree(c->d_kappa); cudaFree(c->d_A); cudaFree(c->d_src_g); cudaFree(c->d_src_S);
     cudaFree(c->d_stacks); cudaFree(c->d_queue); cudaFree(c->d_qseq);
     for (int i = 0; i < 8; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
@@ -113,6 +114,9 @@ int arc_set_params(arc_ctx *c, const arc_params *p)
     if (p->trace_blocks < 0) return fail(c, ARC_EINVAL, "arc_set_params: trace_blocks must be >= 0");
     if (p->deposit < ARC_DEPOSIT_AUTO || p->deposit > ARC_DEPOSIT_QUAD) return fail(c, ARC_EINVAL, "arc_set_params: bad deposit mode");
     if (p->geom_corr < ARC_GEOM_NONE || p->geom_corr > ARC_GEOM_FC2) return fail(c, ARC_EINVAL, "arc_set_params: bad geom_corr");
+    if (!(p->thin_tau >= 0.0) || !std::isfinite(p->thin_tau)) return fail(c, ARC_EINVAL, "arc_set_params: thin_tau must be finite and >= 0");
+    if (p->thin_tau > 0.0 && (p->geom_corr != ARC_GEOM_NONE || p->deposit != ARC_DEPOSIT_AUTO))
+        return fail(c, ARC_EINVAL, "arc_set_params: the optically thin region is built for deposit = AUTO and geom_corr = NONE only");
     if (p->geom_corr != ARC_GEOM_NONE && p->deposit != ARC_DEPOSIT_AUTO)
         return fail(c, ARC_EINVAL, "arc_set_params: the geometric correction is built for deposit = ARC_DEPOSIT_AUTO only");
     c->p = *p;
@@ -210,6 +214,8 @@ int arc_set_sources(arc_ctx *c, int nsrc, const double *pos_cm, const double *Nd
     cudaFree(c->d_src_g); cudaFree(c->d_src_S); c->d_src_g = nullptr; c->d_src_S = nullptr;
     cudaFree(c->d_blocked); c->d_blocked = nullptr; c->mask_level = -1;
     c->h_src_S = S;
+    c->h_R.assign((size_t)nsrc, 0.0);
+    c->h_nopen.assign((size_t)nsrc, -1.0);         // (-1: no mask, all root rays open)
     if (nsrc > 0) {
         CK(cudaMalloc(&c->d_src_g, g.size() * sizeof(double)));
         CK(cudaMalloc(&c->d_src_S, S.size() * sizeof(double)));
@@ -218,6 +224,27 @@ int arc_set_sources(arc_ctx *c, int nsrc, const double *pos_cm, const double *Nd
     }
     c->nsrc = nsrc;
     c->have_src = true;
+    c->have_rates = false;
+    return ARC_OK;
+}
+
+int arc_get_thin_radii(arc_ctx *c, double *R_cells)
+{
+    if (!c) return ARC_EINVAL;
+    if (!c->have_src) return fail(c, ARC_ESTATE, "arc_get_thin_radii: no sources set");
+    if (!R_cells && c->nsrc > 0) return fail(c, ARC_EINVAL, "arc_get_thin_radii: NULL argument");
+    for (int s = 0; s < c->nsrc; ++s) R_cells[s] = c->h_R[(size_t)s];
+    return ARC_OK;
+}
+
+int arc_set_thin_radii(arc_ctx *c, const double *R_cells)
+{
+    if (!c) return ARC_EINVAL;
+    if (!c->have_src) return fail(c, ARC_ESTATE, "arc_set_thin_radii: no sources set");
+    if (!R_cells && c->nsrc > 0) return fail(c, ARC_EINVAL, "arc_set_thin_radii: NULL argument");
+    for (int s = 0; s < c->nsrc; ++s)
+        if (!(R_cells[s] >= 0.0) || !std::isfinite(R_cells[s])) return fail(c, ARC_EINVAL, "arc_set_thin_radii: radii must be finite and >= 0");
+    for (int s = 0; s < c->nsrc; ++s) c->h_R[(size_t)s] = R_cells[s];
     c->have_rates = false;
     return ARC_OK;
 }
@@ -231,6 +258,7 @@ int arc_set_emission_mask(arc_ctx *c, const uint8_t *blocked, int level)
     cudaFree(c->d_blocked); c->d_blocked = nullptr; c->mask_level = -1;
     for (int v = 0; v < ARC_MAX_BINS; ++v) c->emitted[v] = 0.0;
     if (!blocked) {
+        c->h_nopen.assign((size_t)c->nsrc, -1.0);
         for (int s = 0; s < c->nsrc; ++s) for (int v = 0; v < nb; ++v) c->emitted[v] += c->h_src_S[(size_t)s * nb + v];
         c->have_rates = false;
         return ARC_OK;
@@ -240,6 +268,7 @@ int arc_set_emission_mask(arc_ctx *c, const uint8_t *blocked, int level)
     for (int s = 0; s < c->nsrc; ++s) {
         size_t nopen = npix0;
         for (size_t p = 0; p < npix0; ++p) if (blocked[(size_t)s * npix0 + p]) --nopen;
+        c->h_nopen[(size_t)s] = (double)nopen;
         for (int v = 0; v < nb; ++v) c->emitted[v] += c->h_src_S[(size_t)s * nb + v] / (double)npix0 * (double)nopen;
     }
     if (c->nsrc > 0) {

@@ -109,6 +109,57 @@ cudaError_t arc_launch_opacity(arc_ctx *c)
     return cudaGetLastError();
 }
 
+// Optically thin inner region (PAPER.md:116-130 (iii); readings G33-G37): for every source with Rstart > 0, each cell
+// whose centre lies within Rstart receives S_nu kappa_nu V / (4 pi r^2) absorbed photons/s (Eq. 1 for small tau with the
+// dilution 4 pi r^2; r^2 not below (d/2)^2).  blockIdx.y = source, blockIdx.x/threadIdx.x = cell of the cube of side
+// 2 ceil(maxR) + 1 around the source's cell.  Membership (d2 <= R^2) is contract arithmetic in the oracle's order.
+template <typename FT>
+__global__ void __launch_bounds__(256) arc_thin_region_kernel(int N, int nsrc, int nb, int nbp, int side, double dx, const double *__restrict__ src_g,
+                                                             const double *__restrict__ Rstart, const double *__restrict__ Sopen,
+                                                             const FT *__restrict__ kappa, double *__restrict__ A)
+{
+  for (int s = blockIdx.y; s < nsrc; s += gridDim.y) {
+    const double R = Rstart[s];
+    if (!(R > 0.0)) continue;
+    const double gx = src_g[3 * s], gy = src_g[3 * s + 1], gz = src_g[3 * s + 2];
+    const int h = side / 2;
+    const int cx = (int)floor(gx), cy = (int)floor(gy), cz = (int)floor(gz);
+    const double R2 = __dmul_rn(R, R);
+    const double PI = 3.14159265358979323846;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < (long long)side * side * side; t += (long long)gridDim.x * blockDim.x) {
+        const int ix = cx - h + (int)(t % side), iy = cy - h + (int)((t / side) % side), iz = cz - h + (int)(t / ((long long)side * side));
+        if ((unsigned)ix >= (unsigned)N || (unsigned)iy >= (unsigned)N || (unsigned)iz >= (unsigned)N) continue;
+        const double ex = __dsub_rn(__dadd_rn((double)ix, 0.5), gx), ey = __dsub_rn(__dadd_rn((double)iy, 0.5), gy), ez = __dsub_rn(__dadd_rn((double)iz, 0.5), gz);
+        const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+        if (!(d2 <= R2)) continue;
+        const double r2 = d2 < 0.25 ? 0.25 : d2;
+        const long long c = ((long long)iz * N + iy) * N + ix;
+        for (int v = 0; v < nb; ++v) {
+            const double a_v = Sopen[(size_t)s * nb + v] * ((double)kappa[c * nb + v] * dx) / (4.0 * PI * r2);
+            atomicAdd(A + c * nbp + v, a_v);
+        }
+    }
+  }
+}
+
+cudaError_t arc_launch_thin_region(arc_ctx *c, double maxR)
+{
+    int side = 2 * (int)ceil(maxR) + 3;
+    if (side > 2 * c->N + 1) side = 2 * c->N + 1;
+    const long long cells = (long long)side * side * side;
+    long long gx = (cells + 255) / 256;
+    if (gx > 1024) gx = 1024;
+    const dim3 grid((unsigned)gx, (unsigned)(c->nsrc < 65535 ? c->nsrc : 65535));
+    const int nb = c->spec.nb;
+    if (c->dtype == ARC_F32)
+        arc_thin_region_kernel<float><<<grid, 256, 0, c->stream>>>(c->N, c->nsrc, nb, arc_nbp(nb), side, c->dx, c->d_src_g, c->d_Rstart, c->d_Sopen,
+                                                                  (const float *)c->d_kappa, c->d_A);
+    else
+        arc_thin_region_kernel<double><<<grid, 256, 0, c->stream>>>(c->N, c->nsrc, nb, arc_nbp(nb), side, c->dx, c->d_src_g, c->d_Rstart, c->d_Sopen,
+                                                                   (const double *)c->d_kappa, c->d_A);
+    return cudaGetLastError();
+}
+
 cudaError_t arc_launch_finalize(arc_ctx *c)
 {
     cudaError_t e = cudaMemsetAsync(c->d_absorbed, 0, sizeof(double) * ARC_MAX_BINS, c->stream);

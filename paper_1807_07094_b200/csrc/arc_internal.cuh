@@ -73,6 +73,12 @@ struct TraceArgs {
     const double *src_g;       // [nsrc][3] source position in grid units
     const double *src_S;       // [nsrc][nb] Ndot * binfrac
     const unsigned char *blocked;   // NULL or [nsrc][12 4^l0]: blocked root rays (anisotropic emission)
+    // optically thin inner region: all NULL / 0 when off
+    double thin_tau;
+    const double *Rstart;               // [nsrc] start radius of the root rays (cells)
+    unsigned long long *Rnext;          // [nsrc] bits of the radius found by this trace (atomicMin; starts at +inf)
+    const unsigned long long *seed_prefix;   // [nsrc + 1] first root family of each source
+    const int *src_level;               // [nsrc] level of each source's root rays
     unsigned char *stacks;     // n_warps * ARC_STACK_CAP family records
     unsigned char *queue;      // ARC_QUEUE_CAP family records
     unsigned long long *qseq;  // ARC_QUEUE_CAP slot sequence numbers
@@ -105,6 +111,11 @@ struct arc_ctx {
     double *d_src_g = 0, *d_src_S = 0;
     std::vector<double> h_src_S;      // host copy of Ndot * binfrac (emitted with an emission mask)
     unsigned char *d_blocked = 0; int mask_level = -1;     // arc_set_emission_mask
+    std::vector<double> h_nopen;      // open root rays per source (emission mask), npix0 without a mask
+    // optically thin inner region (arc_params.thin_tau > 0): radii found by the last trace, and the device arrays of a trace
+    std::vector<double> h_R;
+    double *d_Rstart = 0; unsigned long long *d_Rnext = 0; unsigned long long *d_seed_prefix = 0; int *d_src_level = 0;
+    double *d_Sopen = 0; int thin_cap = 0;
     double emitted[ARC_MAX_BINS];
     void *d_kappa = 0; int kappa_nb = 0;
     double *d_A = 0; int A_nb = 0;
@@ -125,6 +136,7 @@ struct arc_ctx {
 // arc_fields.cu
 cudaError_t arc_launch_opacity(arc_ctx *c);
 cudaError_t arc_launch_finalize(arc_ctx *c);
+cudaError_t arc_launch_thin_region(arc_ctx *c, double maxR);     // inner-region deposit for the sources with Rstart > 0
 // arc_trace.cu
 cudaError_t arc_launch_sched_reset(arc_ctx *c, unsigned long long seed_total);
 cudaError_t arc_launch_trace(arc_ctx *c, const TraceArgs &a, bool log, int *grid_out);

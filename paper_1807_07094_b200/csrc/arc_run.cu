@@ -44,7 +44,9 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
     if (c->d_blocked && c->mask_level != c->p.l0) return fail(c, ARC_ESTATE, "arc_trace: the emission mask was set for another l0 (arc_set_emission_mask)");
     const int nb = c->spec.nb;
     // persistent grid: what is co-resident (SM count x blocks per SM), or the caller's override
-    const int flags = (log ? 3 : (c->p.digest ? 2 : 0)) | (c->p.geom_corr ? 4 : 0);     // FLAG_LOG 1, FLAG_DIGEST 2, FLAG_GEOM 4
+    const bool thin = c->p.thin_tau > 0.0;
+    if (thin && log) return fail(c, ARC_EINVAL, "arc_trace_debug: the per-ray log is not built for thin_tau > 0");
+    const int flags = (log ? 3 : (c->p.digest ? 2 : 0)) | (c->p.geom_corr ? 4 : 0) | (thin ? 8 : 0);     // FLAG_LOG 1, FLAG_DIGEST 2, FLAG_GEOM 4, FLAG_THIN 8
     const int resident = arc_trace_occupancy_grid(c, nb, flags);
     int grid = c->p.trace_blocks > 0 ? c->p.trace_blocks : resident;
     if (grid > resident) grid = resident;         // blocks wait on one another: never oversubscribe
@@ -79,6 +81,46 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
     a.stacks = c->d_stacks; a.queue = c->d_queue; a.qseq = c->d_qseq; a.sched = c->d_sched; a.stats = c->d_stats;
     a.fam_per_src = 3u << (2 * c->p.l0);
     a.seed_total = (unsigned long long)c->nsrc * a.fam_per_src;
+    double thin_maxR = 0.0;
+    if (thin && c->nsrc > 0) {
+        // optically thin inner region: per source, the radius the last trace found, the level rays have
+        // there (r_split(l-1) <= R < r_split(l)), its root families, and the rate the open root rays carry together
+        const int ns = c->nsrc;
+        if (c->thin_cap < ns) {
+            CK(cudaStreamSynchronize(c->stream));
+            cudaFree(c->d_Rstart); cudaFree(c->d_Rnext); cudaFree(c->d_seed_prefix); cudaFree(c->d_src_level); cudaFree(c->d_Sopen);
+            c->d_Rstart = nullptr; c->d_Rnext = nullptr; c->d_seed_prefix = nullptr; c->d_src_level = nullptr; c->d_Sopen = nullptr; c->thin_cap = 0;
+            CK(cudaMalloc(&c->d_Rstart, sizeof(double) * ns));
+            CK(cudaMalloc(&c->d_Rnext, sizeof(unsigned long long) * ns));
+            CK(cudaMalloc(&c->d_seed_prefix, sizeof(unsigned long long) * (ns + 1)));
+            CK(cudaMalloc(&c->d_src_level, sizeof(int) * ns));
+            CK(cudaMalloc(&c->d_Sopen, sizeof(double) * ns * ARC_MAX_BINS));
+            c->thin_cap = ns;
+        }
+        std::vector<unsigned long long> prefix((size_t)ns + 1), inf((size_t)ns, 0x7ff0000000000000ull);
+        std::vector<int> lev((size_t)ns);
+        std::vector<double> Sopen((size_t)ns * nb);
+        const double npix0 = (double)(12ull << (2 * c->p.l0));
+        prefix[0] = 0;
+        for (int s = 0; s < ns; ++s) {
+            const double R = c->h_R[(size_t)s];
+            int l = c->p.l0;
+            if (R > 0.0) while (l < c->p.Lmax && std::ldexp(a.csplit, l) <= R) ++l;
+            lev[(size_t)s] = l;
+            prefix[(size_t)s + 1] = prefix[(size_t)s] + (3ull << (2 * l));
+            if (R > thin_maxR) thin_maxR = R;
+            const double nopen = c->h_nopen[(size_t)s] < 0.0 ? npix0 : c->h_nopen[(size_t)s];
+            for (int v = 0; v < nb; ++v) Sopen[(size_t)s * nb + v] = c->h_src_S[(size_t)s * nb + v] / npix0 * nopen;
+        }
+        CK(cudaMemcpyAsync(c->d_Rstart, c->h_R.data(), sizeof(double) * ns, cudaMemcpyHostToDevice, c->stream));
+        CK(cudaMemcpyAsync(c->d_Rnext, inf.data(), sizeof(unsigned long long) * ns, cudaMemcpyHostToDevice, c->stream));
+        CK(cudaMemcpyAsync(c->d_seed_prefix, prefix.data(), sizeof(unsigned long long) * (ns + 1), cudaMemcpyHostToDevice, c->stream));
+        CK(cudaMemcpyAsync(c->d_src_level, lev.data(), sizeof(int) * ns, cudaMemcpyHostToDevice, c->stream));
+        CK(cudaMemcpyAsync(c->d_Sopen, Sopen.data(), sizeof(double) * ns * nb, cudaMemcpyHostToDevice, c->stream));
+        CK(cudaStreamSynchronize(c->stream));                        // (the host vectors go out of scope)
+        a.thin_tau = c->p.thin_tau; a.Rstart = c->d_Rstart; a.Rnext = c->d_Rnext; a.seed_prefix = c->d_seed_prefix; a.src_level = c->d_src_level;
+        a.seed_total = prefix[(size_t)ns];
+    }
     {   // few sources: spread the root families over the warps instead of 8 per warp
         const unsigned long long per_warp = a.seed_total / ((unsigned long long)grid * ARC_WARPS_PER_BLOCK);
         a.seed_chunk = per_warp >= ARC_BATCH_FAM ? ARC_BATCH_FAM : (per_warp < 1 ? 1 : (int)per_warp);
@@ -89,6 +131,7 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
     CK(cudaEventRecord(c->ev[0], c->stream));
     CK(arc_launch_sched_reset(c, a.seed_total));
     CK(arc_launch_opacity(c));
+    if (thin && thin_maxR > 0.0) CK(arc_launch_thin_region(c, thin_maxR));          // (iii): after the accumulators are zeroed
     CK(cudaEventRecord(c->ev[1], c->stream));
     CK(arc_launch_trace(c, a, log != nullptr, nullptr));
     CK(cudaEventRecord(c->ev[2], c->stream));
@@ -96,6 +139,19 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
     CK(cudaEventRecord(c->ev[3], c->stream));
     c->traced_once = true;
     c->have_rates = true;
+    if (thin && c->nsrc > 0) {                 // (ii): the radii this trace found are the next trace's
+        std::vector<unsigned long long> bits((size_t)c->nsrc);
+        CK(cudaMemcpyAsync(bits.data(), c->d_Rnext, sizeof(unsigned long long) * c->nsrc, cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaStreamSynchronize(c->stream));
+        const int de = device_error(c);
+        if (de != ARC_OK) return de;
+        for (int s = 0; s < c->nsrc; ++s) {
+            double R = 0.0;
+            if (bits[(size_t)s] < 0x7ff0000000000000ull) std::memcpy(&R, &bits[(size_t)s], sizeof(R));
+            c->h_R[(size_t)s] = R;
+        }
+        return ARC_OK;
+    }
     if (!c->p.async || log) {
         CK(cudaStreamSynchronize(c->stream));
         return device_error(c);

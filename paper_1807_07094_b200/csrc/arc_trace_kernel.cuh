@@ -29,6 +29,7 @@
 #define FLAG_LOG 1          // template flag: per-ray logging (arc_trace_debug)
 #define FLAG_DIGEST 2       // template flag: accumulate the order-independent traversal digest
 #define FLAG_GEOM 4         // template flag: geometric correction of the deposit (Eq. 2-3), mode in TraceArgs::geom
+#define FLAG_THIN 8         // template flag: track, per source, the radius up to which tau (bin 0) stays below thin_tau
 
 #ifndef ARC_TRACE_MIN_BLOCKS
 #define ARC_TRACE_MIN_BLOCKS 3     // resident blocks per SM the register budget is held to (<= 85 registers)
@@ -297,9 +298,19 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                     if (lane < n) {
                         Rec r;
                         const unsigned long long s = s0 + lane;
-                        r.src = (uint32_t)(s / a.fam_per_src); r.fam = (uint32_t)(s % a.fam_per_src);
-                        r.level = (uint32_t)a.l0; r.pad = 0;
-                        const double npix0 = (double)(12ull << (2 * a.l0));
+                        if (a.seed_prefix == nullptr) {
+                            r.src = (uint32_t)(s / a.fam_per_src); r.fam = (uint32_t)(s % a.fam_per_src);
+                            r.level = (uint32_t)a.l0;
+                        } else {
+                            // optically thin start (PAPER.md:130 (iv)): source i owns root families [prefix[i], prefix[i+1]) at its
+                            // own level src_level[i]; binary search for the source
+                            int lo = 0, hi = a.nsrc;                      // prefix[lo] <= s < prefix[hi]
+                            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(a.seed_prefix + mid) <= s) lo = mid; else hi = mid; }
+                            r.src = (uint32_t)lo; r.fam = (uint32_t)(s - __ldg(a.seed_prefix + lo));
+                            r.level = (uint32_t)__ldg(a.src_level + lo);
+                        }
+                        r.pad = 1;                                        // root family: starts at Rstart[src] (0 without a thin region)
+                        const double npix0 = (double)(12ull << (2 * r.level));
 #pragma unroll
                         for (int v = 0; v < NB; ++v) { r.tau[v] = 0.0; r.P[v] = __ldg(a.src_S + (size_t)r.src * NB + v) / npix0; }
                         STK(top + lane) = r;
@@ -338,15 +349,16 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
         double tau[NB], P[NB];
         const double INF = __longlong_as_double(0x7ff0000000000000ll);
         double tx = INF, ty = INF, tz = INF, r = 0, r_end = 0;
+        [[maybe_unused]] double rthin = INF;   // FLAG_THIN: smallest radius at which this lane's ray stopped being optically thin
         unsigned ijk = 0;                      // cell coordinates, 10 bits each (N <= 1024)
         int cell = 0;                          // N <= 1024: N^3 <= 2^30
         int end = -1;
         unsigned long long h = 0; unsigned int seq = 0;
         if (active && a.blocked != nullptr) {                 // anisotropic emission: a blocked root ray does not exist
             const Rec *rp = &STK(top + myfam);
-            if ((int)rp->level == a.l0) {
-                const size_t ip = (size_t)rp->src * ((size_t)12 << (2 * a.l0)) + (4u * rp->fam + (uint32_t)(lane & 3));
-                if (a.blocked[ip]) active = false;
+            if (rp->pad != 0) {                               // (a root above level l0 - thin start - is blocked with its level-l0 ancestor)
+                const uint32_t p0 = (4u * rp->fam + (uint32_t)(lane & 3)) >> (2 * ((int)rp->level - a.l0));
+                if (a.blocked[(size_t)rp->src * ((size_t)12 << (2 * a.l0)) + p0]) active = false;
             }
         }
         if (active) {
@@ -363,7 +375,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
 #define GEO_ST(row, val) asm volatile("st.shared.f64 [%0+%1], %2;" ::"r"(geo_ad), "n"((row) * ARC_TRACE_THREADS * 8), "d"(val))
             GEO_ST(0, gx); GEO_ST(1, gy); GEO_ST(2, gz); GEO_ST(3, dirx); GEO_ST(4, diry); GEO_ST(5, dirz);
             // split radii: exact power-of-two scalings of csplit (O2)
-            r = (level == a.l0) ? 0.0 : scalbn(a.csplit, level - 1);
+            r = rp->pad != 0 ? (a.Rstart != nullptr ? __ldg(a.Rstart + src) : 0.0) : scalbn(a.csplit, level - 1);
             r_end = (level >= a.Lmax) ? INF : scalbn(a.csplit, level);
             // a5: starting cell (O3 step 2)
             const double x0 = arc_add(gx, arc_mul(r, dirx)), y0 = arc_add(gy, arc_mul(r, diry)), z0 = arc_add(gz, arc_mul(r, dirz));
@@ -448,10 +460,14 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                     const unsigned long long yy = arc_mul2(xx, arc_pack2(-1.4426950408889634f, -1.4426950408889634f));
                     arc_unpack2(xx, x[v], x[v + 1]); arc_unpack2(pp, om[v], om[v + 1]); arc_unpack2(yy, y[v], y[v + 1]);
                 }
+                [[maybe_unused]] const double tau0_prev = tau[0];
 #pragma unroll
                 for (int v = 0; v < NB; ++v) {
                     tau[v] = arc_add(tau[v], arc_mul(kcur.get(v), dl));
                     depleted = depleted && (tau[v] >= a.tau_term);       // min_nu tau_nu >= tau_term
+                }
+                if constexpr ((FLAGS & FLAG_THIN) != 0) {                // (ii) of PAPER.md:120: tau reaches thin_tau in this segment,
+                    if (tau0_prev < a.thin_tau && tau[0] >= a.thin_tau) rthin = fmin(rthin, r);     // which starts at radius r
                 }
                 // last use of kcur is above: the NEXT cell's opacities (always a valid cell: no divergence) go straight into
                 // it and have the rest of this iteration, the deposit stage and the next march to arrive
@@ -467,11 +483,15 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                 }
             } else {
                 double dtau[NB];
+                [[maybe_unused]] const double tau0_prev = tau[0];
 #pragma unroll
                 for (int v = 0; v < NB; ++v) {
                     dtau[v] = arc_mul(kcur.get(v), dl);
                     tau[v] = arc_add(tau[v], dtau[v]);
                     depleted = depleted && (tau[v] >= a.tau_term);
+                }
+                if constexpr ((FLAGS & FLAG_THIN) != 0) {
+                    if (tau0_prev < a.thin_tau && tau[0] >= a.thin_tau) rthin = fmin(rthin, r);
                 }
                 kcur.load(kappa, go ? cell_next : cell);       // (as above)
 #pragma unroll
@@ -657,6 +677,14 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
         __syncwarp();
 
         // ------------------------------------------------------------------ a8/a9: bookkeeping, push children
+        if constexpr ((FLAGS & FLAG_THIN) != 0) {
+            // a ray that left the box or was depleted while still thin: thin up to where it ended (r is its final radius)
+            if ((end == ARC_END_ESCAPED || end == ARC_END_DEPLETED) && tau[0] < a.thin_tau) rthin = fmin(rthin, r);
+            if (rthin < INF) {
+                const unsigned long long bits = (unsigned long long)__double_as_longlong(rthin);    // radii >= 0: bits order as values
+                if (bits < ld_volatile_u64(a.Rnext + src)) atomicMin(a.Rnext + src, bits);           // (values only decrease: a stale read is safe)
+            }
+        }
         {
             // a9 tallies, once per batch and warp: rays by end reason (ballots), photons that left the box (warp sum of P
             // over the lanes whose ray escaped; P is untouched once a ray has ended)
@@ -778,6 +806,14 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
 template <int NB, typename KT, int DEP>
 cudaError_t launch_dep(const TraceArgs &a, bool log, int grid, cudaStream_t s)
 {
+    if (a.flags & FLAG_THIN) {                   // AUTO deposit route, no geometric correction, no ray log (arc_set_params / arc_trace_debug check)
+        if constexpr (DEP == (NB >= 3 ? DEP_T : DEP_AGG)) {
+            if (log || (a.flags & FLAG_GEOM)) return cudaErrorInvalidValue;
+            if (a.flags & FLAG_DIGEST) arc_trace_kernel<NB, KT, FLAG_THIN | FLAG_DIGEST, DEP><<<grid, ARC_TRACE_THREADS, 0, s>>>(a);
+            else arc_trace_kernel<NB, KT, FLAG_THIN, DEP><<<grid, ARC_TRACE_THREADS, 0, s>>>(a);
+            return cudaGetLastError();
+        } else return cudaErrorInvalidValue;
+    }
     if (a.flags & FLAG_GEOM) {                   // built for the AUTO deposit route of this bin count only (arc_set_params checks)
         if constexpr (DEP == (NB >= 3 ? DEP_T : DEP_AGG)) {
             if (log) arc_trace_kernel<NB, KT, FLAG_GEOM | FLAG_LOG | FLAG_DIGEST, DEP><<<grid, ARC_TRACE_THREADS, 0, s>>>(a);
@@ -807,6 +843,14 @@ int occ_dep(int flags)
 {
     int nblk = 0;
     cudaError_t e;
+    if (flags & FLAG_THIN) {
+        if constexpr (DEP == (NB >= 3 ? DEP_T : DEP_AGG)) {
+            if (flags & FLAG_DIGEST) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, arc_trace_kernel<NB, KT, FLAG_THIN | FLAG_DIGEST, DEP>, ARC_TRACE_THREADS, 0);
+            else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, arc_trace_kernel<NB, KT, FLAG_THIN, DEP>, ARC_TRACE_THREADS, 0);
+        } else e = cudaErrorInvalidValue;
+        if (e != cudaSuccess) { cudaGetLastError(); return 1; }
+        return nblk < 1 ? 1 : nblk;
+    }
     if (flags & FLAG_GEOM) {
         if constexpr (DEP == (NB >= 3 ? DEP_T : DEP_AGG)) {
             if (flags & FLAG_LOG) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, arc_trace_kernel<NB, KT, FLAG_GEOM | FLAG_LOG | FLAG_DIGEST, DEP>, ARC_TRACE_THREADS, 0);
