@@ -222,6 +222,8 @@ def run_cuda(args):
     extra = {"deposit": args.deposit} if args.deposit else {}
     if args.geom_corr:
         extra["geom_corr"] = args.geom_corr
+    if args.thin_tau:
+        extra["thin_tau"] = args.thin_tau
     cx = arc.Context(w, fields=dev_fields, stream=stream.cuda_stream, **extra)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
     seg_steps, kern_ms, chem_ms, trace_ms, sub_steps, rec_steps = [], [], [], [], [], []
@@ -307,7 +309,7 @@ def run_cuda(args):
             "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, paper_1807_07094_b200/workloads.py)",
             "config": dict(describe(w), parallelism="replicas" if world > 1 else "single-gpu",
                            l2_policy="inputs larger than L2" if (nc * nb * (bytes_seg // nb)) > 126e6 else "working set fits L2 (small config)",
-                           trace_grid_blocks=trace_grid, deposit=args.deposit, geom_corr=args.geom_corr),
+                           trace_grid_blocks=trace_grid, deposit=args.deposit, geom_corr=args.geom_corr, thin_tau=args.thin_tau),
             "e2e": {"value": job_throughput(e2e_seg_all, e2e_ms_max), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": 5 * args.steps,
             "clocks": clocks,
@@ -353,6 +355,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--geom-corr", type=int, default=0, help="arc_params.geom_corr (PAPER.md:100-114): 0 none (the north_star path), 1 f_c, 2 f_c + secondary, 3 f_c^2")
+    ap.add_argument("--thin-tau", type=float, default=0.0, help="arc_params.thin_tau (PAPER.md:116-130): 0 off (the north_star path), 0.1 in the paper")
     ap.add_argument("--sources", type=int, default=0, help="profiling aid: keep only the first K sources of the workload")
     ap.add_argument("--deposit", type=int, default=0, help="arc_params.deposit: 0 auto, 1 per-lane REDs, 2 warp-aggregated")
     args = ap.parse_args()
