@@ -12,6 +12,7 @@
 // prints only what fixes alpha_B(1e4 K) = 2.59e-13.  The fits below are the published
 // Hui & Gnedin (1997) / Cen (1992) forms, typed here from DESIGN.md "Rate table", in lambda = 2 T_TR / T.
 #include "arc_internal.cuh"
+#include <cmath>
 
 namespace {
 
@@ -23,115 +24,164 @@ struct Coef {
     double cool_ff;                    // bremsstrahlung
 };
 
-// x^a for x > 0 through one log and one exp
-__device__ __forceinline__ double powl_(double lnx, double a) { return exp(a * lnx); }
+// The fits are products of powers of lambda_X = 2 T_X / T.  With L = ln T every such power is a constant times
+// exp(-a L), and species that share an exponent share the exponential; (1 + u)^s = exp(s ln(1 + u)).  The constants
+// (prefactor x (2 T_X)^a, (2 T_X / l0)^q) are evaluated once on the host (chem_consts) and passed by value: one
+// sub-cycle costs 1 log + 1 reciprocal + 1 sqrt + 9 exp + 4 exp/log pairs (+ 8 exp and 3 pairs with collisional
+// ionisation) instead of 16 exp, 4 pow and 4-8 log (25 exp, 7 pow, 4-11 log).  Same functions of T as DESIGN.md 2.1,
+// to a few ulp.
+struct ChemK {
+    double p_rec, q_rec, s_rec, kH_rec, kB_rec, uH_rec, uB_rec;     // alpha_HII(lambda_H), alpha_HeIII = 2 alpha_HII(lambda_HeII)
+    double p_cl, q_cl, s_cl, kH_cl, kB_cl, uH_cl, uB_cl;            // recombination cooling (x T), He III = 8 x at lambda_HeII
+    double p_he, k_he;                                              // alpha_HeII radiative
+    double kcHI, ucHI, kcHeI, ucHeI, kcHeII, ucHeII;                // collisional ionisation
+    int coll, p_rec_is_15;
+};
 
-__device__ void rate_table(double T, bool caseB, bool coll, Coef &k)
+__device__ __forceinline__ void rate_table(double T, const ChemK &q, Coef &k)
 {
     const double KB = 1.380649e-16;
     const double TR_H = 157807.0, TR_HE1 = 285335.0, TR_HE2 = 631515.0;   // ionisation thresholds in K
-    const double lamH = 2.0 * TR_H / T, lamA = 2.0 * TR_HE1 / T, lamB = 2.0 * TR_HE2 / T;
-    const double lnH = log(lamH), lnA = log(lamA), lnB = log(lamB), lnT = log(T);
-    if (caseB) {
-        k.aHII = 2.753e-14 * powl_(lnH, 1.5) / pow(1.0 + powl_(lnH - log(2.74), 0.407), 2.242);
-        k.aHeII = 1.26e-14 * powl_(lnA, 0.75);
-        k.aHeIII = 2.0 * 2.753e-14 * powl_(lnB, 1.5) / pow(1.0 + powl_(lnB - log(2.74), 0.407), 2.242);
-        k.cool_rHII = 3.435e-30 * T * powl_(lnH, 1.97) / pow(1.0 + powl_(lnH - log(2.25), 0.376), 3.72);
-        k.cool_rHeIII = 8.0 * 3.435e-30 * T * powl_(lnB, 1.97) / pow(1.0 + powl_(lnB - log(2.25), 0.376), 3.72);
-    } else {
-        k.aHII = 1.269e-13 * powl_(lnH, 1.503) / pow(1.0 + powl_(lnH - log(0.522), 0.47), 1.923);
-        k.aHeII = 3.0e-14 * powl_(lnA, 0.654);
-        k.aHeIII = 2.0 * 1.269e-13 * powl_(lnB, 1.503) / pow(1.0 + powl_(lnB - log(0.522), 0.47), 1.923);
-        k.cool_rHII = 1.778e-29 * T * powl_(lnH, 1.965) / pow(1.0 + powl_(lnH - log(0.541), 0.502), 2.697);
-        k.cool_rHeIII = 8.0 * 1.778e-29 * T * powl_(lnB, 1.965) / pow(1.0 + powl_(lnB - log(0.541), 0.502), 2.697);
-    }
-    // dielectronic recombination of He II
-    const double Tm15 = exp(-1.5 * lnT);
-    const double adi = 1.9e-3 * Tm15 * exp(-470000.0 / T) * (1.0 + 0.3 * exp(-94000.0 / T));
-    const double aHeII_rad = k.aHeII;
+    const double L = log(T), iT = 1.0 / T;
+    // recombination and its cooling: A0 lambda^p / (1 + (lambda/l0)^q)^s
+    const double ep = exp(-q.p_rec * L), eq = exp(-q.q_rec * L);
+    k.aHII = q.kH_rec * ep * exp(-q.s_rec * log(1.0 + q.uH_rec * eq));
+    k.aHeIII = q.kB_rec * ep * exp(-q.s_rec * log(1.0 + q.uB_rec * eq));
+    const double Tm15 = q.p_rec_is_15 ? ep : exp(-1.5 * L);
+    const double cp = T * exp(-q.p_cl * L), cq = exp(-q.q_cl * L);
+    k.cool_rHII = q.kH_cl * cp * exp(-q.s_cl * log(1.0 + q.uH_cl * cq));
+    k.cool_rHeIII = q.kB_cl * cp * exp(-q.s_cl * log(1.0 + q.uB_cl * cq));
+    // dielectronic recombination of He II: e^{-470000/T} = (e^{-94000/T})^5
+    const double w = exp(-94000.0 * iT), w2 = w * w;
+    const double adi = 1.9e-3 * Tm15 * (w2 * w2 * w) * (1.0 + 0.3 * w);
+    const double aHeII_rad = q.k_he * exp(-q.p_he * L);
     k.aHeII = aHeII_rad + adi;
     k.cool_rHeII = KB * T * aHeII_rad + 6.54e-11 * adi;
     k.cHI = k.cHeI = k.cHeII = 0.0;
-    if (coll) {
-        k.cHI = 21.11 * Tm15 * exp(-0.5 * lamH) * powl_(lnH, -1.089) / pow(1.0 + powl_(lnH - log(0.354), 0.874), 1.101);
-        k.cHeI = 32.38 * Tm15 * exp(-0.5 * lamA) * powl_(lnA, -1.146) / pow(1.0 + powl_(lnA - log(0.416), 0.987), 1.056);
-        k.cHeII = 19.95 * Tm15 * exp(-0.5 * lamB) * powl_(lnB, -1.089) / pow(1.0 + powl_(lnB - log(0.553), 0.735), 1.275);
+    if (q.coll) {   // X T^-1.5 e^{-lambda/2} lambda^-a / (1 + (lambda/l0)^b)^c
+        const double e1089 = exp(1.089 * L);
+        k.cHI = q.kcHI * Tm15 * exp(-TR_H * iT) * e1089 * exp(-1.101 * log(1.0 + q.ucHI * exp(-0.874 * L)));
+        k.cHeI = q.kcHeI * Tm15 * exp(-TR_HE1 * iT) * exp(1.146 * L) * exp(-1.056 * log(1.0 + q.ucHeI * exp(-0.987 * L)));
+        k.cHeII = q.kcHeII * Tm15 * exp(-TR_HE2 * iT) * e1089 * exp(-1.275 * log(1.0 + q.ucHeII * exp(-0.735 * L)));
     }
-    const double damp = 1.0 / (1.0 + sqrt(T / 1.0e5));
-    k.cool_xHI = 7.5e-19 * exp(-118348.0 / T) * damp;
-    k.cool_xHeII = 5.54e-17 * exp(-0.397 * lnT) * exp(-473638.0 / T) * damp;
-    const double u = 5.5 - lnT * 0.43429448190325182765;     // 5.5 - log10 T
-    k.cool_ff = 1.42e-27 * (1.1 + 0.34 * exp(-u * u / 3.0)) * sqrt(T);
+    const double sqT = sqrt(T);
+    const double damp = 1.0 / (1.0 + sqT * 3.1622776601683794e-3);        // 1 / (1 + sqrt(T / 1e5))
+    k.cool_xHI = 7.5e-19 * exp(-118348.0 * iT) * damp;
+    k.cool_xHeII = 5.54e-17 * exp(-0.397 * L - 473638.0 * iT) * damp;
+    const double u = 5.5 - L * 0.43429448190325182765;       // 5.5 - log10 T
+    k.cool_ff = 1.42e-27 * (1.1 + 0.34 * exp(-u * u / 3.0)) * sqT;
+}
+
+// host: the constants of the fits for the chosen recombination case
+static ChemK chem_consts(bool caseB, bool coll)
+{
+    const double LH = 2.0 * 157807.0, LA = 2.0 * 285335.0, LB = 2.0 * 631515.0;
+    ChemK q{};
+    double A0, l0, C0, m0;
+    if (caseB) { A0 = 2.753e-14; q.p_rec = 1.5; l0 = 2.74; q.q_rec = 0.407; q.s_rec = 2.242;
+                 C0 = 3.435e-30; q.p_cl = 1.97; m0 = 2.25; q.q_cl = 0.376; q.s_cl = 3.72; q.k_he = 1.26e-14; q.p_he = 0.75; }
+    else       { A0 = 1.269e-13; q.p_rec = 1.503; l0 = 0.522; q.q_rec = 0.47; q.s_rec = 1.923;
+                 C0 = 1.778e-29; q.p_cl = 1.965; m0 = 0.541; q.q_cl = 0.502; q.s_cl = 2.697; q.k_he = 3.0e-14; q.p_he = 0.654; }
+    q.kH_rec = A0 * std::pow(LH, q.p_rec); q.kB_rec = 2.0 * A0 * std::pow(LB, q.p_rec);
+    q.uH_rec = std::pow(LH / l0, q.q_rec); q.uB_rec = std::pow(LB / l0, q.q_rec);
+    q.kH_cl = C0 * std::pow(LH, q.p_cl); q.kB_cl = 8.0 * C0 * std::pow(LB, q.p_cl);
+    q.uH_cl = std::pow(LH / m0, q.q_cl); q.uB_cl = std::pow(LB / m0, q.q_cl);
+    q.k_he *= std::pow(LA, q.p_he);
+    q.kcHI = 21.11 * std::pow(LH, -1.089); q.ucHI = std::pow(LH / 0.354, 0.874);
+    q.kcHeI = 32.38 * std::pow(LA, -1.146); q.ucHeI = std::pow(LA / 0.416, 0.987);
+    q.kcHeII = 19.95 * std::pow(LB, -1.089); q.ucHeII = std::pow(LB / 0.553, 0.735);
+    q.coll = coll ? 1 : 0; q.p_rec_is_15 = q.p_rec == 1.5 ? 1 : 0;
+    return q;
 }
 
 __device__ __forceinline__ double clamp01(double v, double lo) { return v < lo ? lo : (v > 1.0 ? 1.0 : v); }
 
-template <typename FT, bool ISO>
-__global__ void __launch_bounds__(128) arc_chem_kernel(long long ncell, double dt, double Yp, double eps, double x_floor,
-                                                      int max_sub, int caseB, int coll,
-                                                      const FT *__restrict__ nHf, FT *__restrict__ xHIf, FT *__restrict__ xHeIf,
-                                                      FT *__restrict__ xHeIIf, FT *__restrict__ Tf,
-                                                      const double *__restrict__ rates, DevStats *stats)
+// state of one cell during the sub-cycle loop
+struct Cell {
+    double nH, nHe, x0, x1, x2, T, G0, G1, G2, H0, H1, H2, t;
+    int n;
+};
+
+// one sub-cycle of PAPER.md:136-154 (readings G12, G15-G17, G23, G24); k = rate table at c.T (ISO: evaluated by the caller)
+template <bool ISO>
+__device__ __forceinline__ void chem_subcycle(Cell &c, Coef &k, const ChemK &q, double dt, double eps, double x_floor, int max_sub)
 {
     const double KB = 1.380649e-16;
     // collisional-ionisation cooling = threshold energy x rate (13.6, 24.6, 54.4 eV in erg)
     const double EI_H = 2.18e-11, EI_HE1 = 3.94e-11, EI_HE2 = 8.72e-11;
+    const double nH = c.nH, nHe = c.nHe, x0 = c.x0, x1 = c.x1, x2 = c.x2;
+    const double xHII = 1.0 - x0;
+    double xHeIII = 1.0 - x1 - x2; if (xHeIII < 0.0) xHeIII = 0.0;
+    const double ne = nH * xHII + nHe * (x2 + 2.0 * xHeIII);
+    if (!ISO) rate_table(c.T, q, k);
+    // Eq. 4 written as Eq. 5 (dn/dt = D - C n), in fractions
+    const double C0 = c.G0 + k.cHI * ne,              D0 = k.aHII * ne * xHII;
+    const double C1 = c.G1 + k.cHeI * ne,             D1 = k.aHeII * ne * x2;
+    const double C2 = (c.G2 + k.cHeII * ne) + k.aHeII * ne;
+    const double D2 = (c.G1 + k.cHeI * ne) * x1 + k.aHeIII * ne * xHeIII;
+    double left = dt - c.t, dts = left;
+    double heat = 0.0, cool = 0.0, E = 0.0;
+    if (!ISO) {
+        const double nHI = nH * x0, nHeI = nHe * x1, nHeII = nHe * x2, nHII = nH * xHII, nHeIII = nHe * xHeIII;
+        heat = (c.H0 * nHI + c.H1 * nHeI) + c.H2 * nHeII;
+        cool = ne * (k.cool_rHII * nHII + k.cool_rHeII * nHeII + k.cool_rHeIII * nHeIII
+                     + EI_H * k.cHI * nHI + EI_HE1 * k.cHeI * nHeI + EI_HE2 * k.cHeII * nHeII
+                     + k.cool_xHI * nHI + k.cool_xHeII * nHeII
+                     + k.cool_ff * (nHII + nHeII + 4.0 * nHeIII));
+        E = 1.5 * KB * c.T * (nH + nHe + ne);
+    }
+    if (c.n != max_sub - 1) {
+        const double xdot = D0 - C0 * x0;
+        if (xdot != 0.0) dts = fmin(dts, eps * x0 / fabs(xdot));
+        if (!ISO && heat - cool != 0.0) dts = fmin(dts, eps * E / fabs(heat - cool));
+    }
+    const double y0 = (x0 + D0 * dts) / (1.0 + C0 * dts);                     // Eq. 5 backward difference
+    const double y1 = (x1 + D1 * dts) / (1.0 + C1 * dts);
+    const double y2 = (x2 + D2 * dts) / (1.0 + C2 * dts);
+    c.x0 = clamp01(y0, x_floor); c.x1 = clamp01(y1, x_floor); c.x2 = clamp01(y2, 0.0);
+    if (c.x1 + c.x2 > 1.0) { const double s = c.x1 + c.x2; c.x1 = c.x1 / s; c.x2 = c.x2 / s; }
+    if (!ISO) {
+        const double En = (E + heat * dts) / (1.0 + (cool / E) * dts);
+        double xHeIII_n = 1.0 - c.x1 - c.x2; if (xHeIII_n < 0.0) xHeIII_n = 0.0;
+        const double ne_n = nH * (1.0 - c.x0) + nHe * (c.x2 + 2.0 * xHeIII_n);
+        c.T = fmax(En / (1.5 * KB * (nH + nHe + ne_n)), 1.0);
+    }
+    c.t = (dts >= left) ? dt : c.t + dts;
+    ++c.n;
+}
+
+template <typename FT, bool ISO>
+__device__ __forceinline__ void chem_load(Cell &c, long long i, long long ncell, double Yp, const FT *__restrict__ nHf,
+                                          const FT *__restrict__ xHIf, const FT *__restrict__ xHeIf, const FT *__restrict__ xHeIIf,
+                                          const FT *__restrict__ Tf, const double *__restrict__ rates)
+{
+    c.nH = (double)nHf[i];
+    c.nHe = c.nH * Yp / (4.0 * (1.0 - Yp));
+    c.x0 = (double)xHIf[i]; c.x1 = (double)xHeIf[i]; c.x2 = (double)xHeIIf[i]; c.T = (double)Tf[i];
+    c.G0 = rates[i]; c.G1 = rates[ncell + i]; c.G2 = rates[2 * ncell + i];
+    c.H0 = c.H1 = c.H2 = 0.0;
+    if (!ISO) { c.H0 = rates[3 * ncell + i]; c.H1 = rates[4 * ncell + i]; c.H2 = rates[5 * ncell + i]; }
+    c.t = 0.0; c.n = 0;
+}
+
+// Isothermal runs (configs 1-2): the rate table is evaluated once per cell and a sub-cycle is a few dozen flops, so
+// one thread keeps one cell; fully coalesced grid-stride pass.
+template <typename FT>
+__global__ void __launch_bounds__(128) arc_chem_iso_kernel(long long ncell, double dt, double Yp, double eps, double x_floor,
+                                                          int max_sub, ChemK q,
+                                                          const FT *__restrict__ nHf, FT *__restrict__ xHIf, FT *__restrict__ xHeIf,
+                                                          FT *__restrict__ xHeIIf, FT *__restrict__ Tf,
+                                                          const double *__restrict__ rates, DevStats *stats)
+{
     unsigned long long my_sub = 0; unsigned int my_max = 0;
-    for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
-        const double nH = (double)nHf[c];
-        const double nHe = nH * Yp / (4.0 * (1.0 - Yp));
-        double x0 = (double)xHIf[c], x1 = (double)xHeIf[c], x2 = (double)xHeIIf[c], T = (double)Tf[c];
-        const double G0 = rates[c], G1 = rates[ncell + c], G2 = rates[2 * ncell + c];
-        double H0 = 0.0, H1 = 0.0, H2 = 0.0;
-        if (!ISO) { H0 = rates[3 * ncell + c]; H1 = rates[4 * ncell + c]; H2 = rates[5 * ncell + c]; }
-        Coef k;
-        if (ISO) rate_table(T, caseB != 0, coll != 0, k);
-        double t = 0.0;
-        int n = 0;
-        while (t < dt && n < max_sub) {
-            const double xHII = 1.0 - x0;
-            double xHeIII = 1.0 - x1 - x2; if (xHeIII < 0.0) xHeIII = 0.0;
-            const double ne = nH * xHII + nHe * (x2 + 2.0 * xHeIII);
-            if (!ISO) rate_table(T, caseB != 0, coll != 0, k);
-            // Eq. 4 written as Eq. 5 (dn/dt = D - C n), in fractions
-            const double C0 = G0 + k.cHI * ne,              D0 = k.aHII * ne * xHII;
-            const double C1 = G1 + k.cHeI * ne,             D1 = k.aHeII * ne * x2;
-            const double C2 = (G2 + k.cHeII * ne) + k.aHeII * ne;
-            const double D2 = (G1 + k.cHeI * ne) * x1 + k.aHeIII * ne * xHeIII;
-            double left = dt - t, dts = left;
-            double heat = 0.0, cool = 0.0, E = 0.0;
-            if (!ISO) {
-                const double nHI = nH * x0, nHeI = nHe * x1, nHeII = nHe * x2, nHII = nH * xHII, nHeIII = nHe * xHeIII;
-                heat = (H0 * nHI + H1 * nHeI) + H2 * nHeII;
-                cool = ne * (k.cool_rHII * nHII + k.cool_rHeII * nHeII + k.cool_rHeIII * nHeIII
-                             + EI_H * k.cHI * nHI + EI_HE1 * k.cHeI * nHeI + EI_HE2 * k.cHeII * nHeII
-                             + k.cool_xHI * nHI + k.cool_xHeII * nHeII
-                             + k.cool_ff * (nHII + nHeII + 4.0 * nHeIII));
-                E = 1.5 * KB * T * (nH + nHe + ne);
-            }
-            if (n != max_sub - 1) {
-                const double xdot = D0 - C0 * x0;
-                if (xdot != 0.0) dts = fmin(dts, eps * x0 / fabs(xdot));
-                if (!ISO && heat - cool != 0.0) dts = fmin(dts, eps * E / fabs(heat - cool));
-            }
-            const double y0 = (x0 + D0 * dts) / (1.0 + C0 * dts);                     // Eq. 5 backward difference
-            const double y1 = (x1 + D1 * dts) / (1.0 + C1 * dts);
-            const double y2 = (x2 + D2 * dts) / (1.0 + C2 * dts);
-            x0 = clamp01(y0, x_floor); x1 = clamp01(y1, x_floor); x2 = clamp01(y2, 0.0);
-            if (x1 + x2 > 1.0) { const double s = x1 + x2; x1 = x1 / s; x2 = x2 / s; }
-            if (!ISO) {
-                const double En = (E + heat * dts) / (1.0 + (cool / E) * dts);
-                double xHeIII_n = 1.0 - x1 - x2; if (xHeIII_n < 0.0) xHeIII_n = 0.0;
-                const double ne_n = nH * (1.0 - x0) + nHe * (x2 + 2.0 * xHeIII_n);
-                T = fmax(En / (1.5 * KB * (nH + nHe + ne_n)), 1.0);
-            }
-            t = (dts >= left) ? dt : t + dts;
-            ++n;
-        }
-        xHIf[c] = (FT)x0; xHeIf[c] = (FT)x1; xHeIIf[c] = (FT)x2;
-        if (!ISO) Tf[c] = (FT)T;
-        my_sub += (unsigned long long)n;
-        my_max = max(my_max, (unsigned int)n);
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < ncell; i += (long long)gridDim.x * blockDim.x) {
+        Cell c; Coef k;
+        chem_load<FT, true>(c, i, ncell, Yp, nHf, xHIf, xHeIf, xHeIIf, Tf, rates);
+        rate_table(c.T, q, k);
+        while (c.t < dt && c.n < max_sub) chem_subcycle<true>(c, k, q, dt, eps, x_floor, max_sub);
+        xHIf[i] = (FT)c.x0; xHeIf[i] = (FT)c.x1; xHeIIf[i] = (FT)c.x2;
+        my_sub += (unsigned long long)c.n;
+        my_max = max(my_max, (unsigned int)c.n);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -141,12 +191,63 @@ __global__ void __launch_bounds__(128) arc_chem_kernel(long long ncell, double d
     if ((threadIdx.x & 31) == 0) { atomicAdd(&stats->subcycles, my_sub); atomicMax(&stats->max_sub, my_max); }
 }
 
+// Evolving temperature: every sub-cycle re-evaluates the rate table (a few thousand fp64 instructions) and the number of
+// sub-cycles per cell runs from 1 (most of the box) to max_sub (ionisation fronts), so a lane that kept its cell until
+// the slowest cell of the warp finished would idle most of the time.  Persistent warps instead: every lane owns one
+// cell; each warp iteration runs ONE sub-cycle on every lane, and lanes whose cell is finished write it back and take
+// the next cells from a global counter (one atomicAdd per warp and refill) - all 32 lanes stay busy until the grid is
+// used up.  The arithmetic per cell is exactly that of the one-thread-per-cell loop.
+template <typename FT>
+__global__ void __launch_bounds__(128) arc_chem_kernel(long long ncell, double dt, double Yp, double eps, double x_floor,
+                                                      int max_sub, ChemK q,
+                                                      const FT *__restrict__ nHf, FT *__restrict__ xHIf, FT *__restrict__ xHeIf,
+                                                      FT *__restrict__ xHeIIf, FT *__restrict__ Tf,
+                                                      const double *__restrict__ rates, DevStats *stats)
+{
+    const unsigned lane = threadIdx.x & 31u;
+    unsigned long long my_sub = 0; unsigned int my_max = 0;
+    long long mine = -1;                          // this lane's cell, -1 = none
+    bool drained = false;                         // warp-uniform: the counter has passed ncell
+    Cell c; Coef k;
+    c.n = 0; c.t = 0.0;
+    for (;;) {
+        const unsigned idle = __ballot_sync(0xffffffffu, mine < 0);
+        if (idle != 0u && !drained) {
+            const int want = __popc(idle);
+            long long base = 0;
+            if (lane == 0) base = (long long)atomicAdd(&stats->chem_next, (unsigned long long)want);
+            base = __shfl_sync(0xffffffffu, base, 0);
+            drained = base + want >= ncell;
+            if (mine < 0) {
+                const long long i = base + __popc(idle & ((1u << lane) - 1u));
+                if (i < ncell) { mine = i; chem_load<FT, false>(c, i, ncell, Yp, nHf, xHIf, xHeIf, xHeIIf, Tf, rates); }
+            }
+        }
+        if (__all_sync(0xffffffffu, mine < 0)) break;
+        if (mine >= 0) {
+            if (c.t < dt && c.n < max_sub) chem_subcycle<false>(c, k, q, dt, eps, x_floor, max_sub);
+            if (!(c.t < dt && c.n < max_sub)) {
+                xHIf[mine] = (FT)c.x0; xHeIf[mine] = (FT)c.x1; xHeIIf[mine] = (FT)c.x2; Tf[mine] = (FT)c.T;
+                my_sub += (unsigned long long)c.n;
+                my_max = max(my_max, (unsigned int)c.n);
+                mine = -1;
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        my_sub += __shfl_xor_sync(0xffffffffu, my_sub, o);
+        my_max = max(my_max, __shfl_xor_sync(0xffffffffu, my_max, o));
+    }
+    if (lane == 0) { atomicAdd(&stats->subcycles, my_sub); atomicMax(&stats->max_sub, my_max); }
+}
+
 // Radiative-transfer time step (include/arc.h arc_suggest_dt): one streaming pass, 28 B per cell
 // (five fields at the field dtype + Gamma_HI), minimum by warp shuffles and one 64-bit atomicMin per warp on the bits of
 // the (positive) double.  The tau > 0.5 test is products only, in the oracle's order: the same cells qualify.
 template <typename FT>
 __global__ void __launch_bounds__(256) arc_dt_kernel(long long ncell, int scheme, double eps, double sigma1, double d, double Yp,
-                                                    int caseB, int coll, const FT *__restrict__ nHf, const FT *__restrict__ xHIf,
+                                                    ChemK q, const FT *__restrict__ nHf, const FT *__restrict__ xHIf,
                                                     const FT *__restrict__ xHeIf, const FT *__restrict__ xHeIIf, const FT *__restrict__ Tf,
                                                     const double *__restrict__ GammaHI, unsigned long long *out)
 {
@@ -159,7 +260,7 @@ __global__ void __launch_bounds__(256) arc_dt_kernel(long long ncell, int scheme
         double xHeIII = 1.0 - x1 - x2; if (xHeIII < 0.0) xHeIII = 0.0;
         const double ne = nH * xHII + nHe * (x2 + 2.0 * xHeIII);
         Coef k;
-        rate_table((double)Tf[c], caseB != 0, coll != 0, k);
+        rate_table((double)Tf[c], q, k);
         const double C0 = GammaHI[c] + k.cHI * ne, D0 = k.aHII * ne * xHII;
         const double nHI = __dmul_rn(nH, x0);
         const double ndot = fabs(nH * (D0 - C0 * x0));
@@ -190,24 +291,30 @@ cudaError_t launch_dt(arc_ctx *c, int scheme, double eps)
     const long long nb = (c->ncell + 255) / 256;
     const long long cap = (long long)c->n_sm * 8;
     FT **f = reinterpret_cast<FT **>(c->f);
-    arc_dt_kernel<FT><<<(int)(nb < cap ? nb : cap), 256, 0, c->stream>>>(c->ncell, scheme, eps, c->spec.sig[0][0], c->dx, c->p.Yp, c->p.caseB,
-                                                                        c->p.coll_ion, f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_dt);
+    arc_dt_kernel<FT><<<(int)(nb < cap ? nb : cap), 256, 0, c->stream>>>(c->ncell, scheme, eps, c->spec.sig[0][0], c->dx, c->p.Yp,
+                                                                        chem_consts(c->p.caseB != 0, c->p.coll_ion != 0), f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_dt);
     return cudaGetLastError();
 }
 
 template <typename FT>
 cudaError_t launch_chem(arc_ctx *c, double dt)
 {
-    const long long nb = (c->ncell + 127) / 128;
-    const long long cap = (long long)c->n_sm * 32;
-    const int grid = (int)(nb < cap ? nb : cap);
     FT **f = reinterpret_cast<FT **>(c->f);
-    if (c->p.isothermal)
-        arc_chem_kernel<FT, true><<<grid, 128, 0, c->stream>>>(c->ncell, dt, c->p.Yp, c->p.eps_sub, c->p.x_floor, c->p.max_subcycles,
-                                                              c->p.caseB, c->p.coll_ion, f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_stats);
-    else
-        arc_chem_kernel<FT, false><<<grid, 128, 0, c->stream>>>(c->ncell, dt, c->p.Yp, c->p.eps_sub, c->p.x_floor, c->p.max_subcycles,
-                                                               c->p.caseB, c->p.coll_ion, f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_stats);
+    const ChemK q = chem_consts(c->p.caseB != 0, c->p.coll_ion != 0);
+    const long long nb = (c->ncell + 127) / 128;
+    if (c->p.isothermal) {
+        const long long cap = (long long)c->n_sm * 32;
+        arc_chem_iso_kernel<FT><<<(int)(nb < cap ? nb : cap), 128, 0, c->stream>>>(c->ncell, dt, c->p.Yp, c->p.eps_sub, c->p.x_floor, c->p.max_subcycles,
+                                                                                 q, f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_stats);
+    } else {
+        // persistent: exactly the co-resident blocks (stats->chem_next is zeroed by arc_update_chemistry)
+        int per_sm = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, arc_chem_kernel<FT>, 128, 0);
+        if (e != cudaSuccess) return e;
+        const long long cap = (long long)c->n_sm * (per_sm > 0 ? per_sm : 1);
+        arc_chem_kernel<FT><<<(int)(nb < cap ? nb : cap), 128, 0, c->stream>>>(c->ncell, dt, c->p.Yp, c->p.eps_sub, c->p.x_floor, c->p.max_subcycles,
+                                                                             q, f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_stats);
+    }
     return cudaGetLastError();
 }
 

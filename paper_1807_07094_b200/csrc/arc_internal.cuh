@@ -52,6 +52,7 @@ struct DevStats {
     unsigned long long subcycles;
     unsigned int max_sub;
     unsigned int pad;
+    unsigned long long chem_next;      // arc_chem_kernel's cell counter (zeroed with the two fields above)
 };
 
 // stride (in doubles) of one cell's accumulators: nb rounded up to even (nb > 1) so that a cell's record is a

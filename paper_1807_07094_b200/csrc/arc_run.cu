@@ -241,7 +241,7 @@ int arc_update_chemistry(arc_ctx *c, double dt_s)
     if (!(dt_s >= 0.0) || !std::isfinite(dt_s)) return fail(c, ARC_EINVAL, "arc_update_chemistry: dt must be finite and >= 0");
     if (!c->have_rates) return fail(c, ARC_ESTATE, "arc_update_chemistry: no valid rates (call arc_trace after setting fields)");
     CK(cudaEventRecord(c->ev[5], c->stream));
-    CK(cudaMemsetAsync(&c->d_stats->subcycles, 0, sizeof(unsigned long long) + 2 * sizeof(unsigned int), c->stream));
+    CK(cudaMemsetAsync(&c->d_stats->subcycles, 0, 2 * sizeof(unsigned long long) + 2 * sizeof(unsigned int), c->stream));
     CK(arc_launch_chemistry(c, dt_s));
     CK(cudaEventRecord(c->ev[6], c->stream));
     c->chem_once = true;
