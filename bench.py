@@ -188,7 +188,7 @@ def job_throughput(units_all_ranks, ms_max_over_ranks):
 def run_cuda(args):
     import torch
     import torch.distributed as dist
-    from paper_1807_07094_b200 import arc
+    from paper_1807_07094_b200 import arc, sharded
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -225,19 +225,27 @@ def run_cuda(args):
     if args.thin_tau:
         extra["thin_tau"] = args.thin_tau
     cx = arc.Context(w, fields=dev_fields, stream=stream.cuda_stream, **extra)
+    shard = args.shard == "sources"
+    my_sources = sharded.partition_sources(w.nsrc, world)[rank] if shard else None
+    if shard:
+        cx.set_sources(my_sources)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
     seg_steps, kern_ms, chem_ms, trace_ms, sub_steps, rec_steps = [], [], [], [], [], []
 
     def one_step(i, record):
-        cx.trace(i)
+        if shard:
+            sharded.trace_sharded(cx, None, i)    # this rank's sources, all-reduce of the accumulators, finalize
+        else:
+            cx.trace(i)
         cx.update_chemistry()
         if record:
             st = cx.stats()                       # synchronises the stream; reads the per-kernel event times
             seg_steps.append(st["segments"]); kern_ms.append(st["trace_kernel_ms"]); chem_ms.append(st["chem_ms"])
             trace_ms.append(st["trace_ms"]); sub_steps.append(st["subcycles"]); rec_steps.append(st["deposit_records"])
 
-    for i in range(args.warmup):
-        one_step(i, False)
+    with torch.cuda.stream(stream):               # (the all-reduce of --shard sources goes to torch's current stream)
+        for i in range(args.warmup):
+            one_step(i, False)
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
     t_host0 = time.perf_counter()
@@ -251,6 +259,10 @@ def run_cuda(args):
     clocks = sampler.stop() if sampler else None
     dev_ms = ev[0].elapsed_time(ev[1])
     cons = cx.stats()
+    if shard:
+        with torch.cuda.stream(stream):
+            cons = sharded.reduce_stats(cons)
+        cons = {k: (np.asarray(v) if isinstance(v, list) else v) for k, v in cons.items()}
     conservation = float(np.max(np.abs((cons["absorbed"] + cons["escaped"]) / cons["emitted"] - 1.0)))
     trace_grid = cons["trace_grid"]
     cx.close()
@@ -260,6 +272,8 @@ def run_cuda(args):
     seg_per_record = None
     if rank == 0:
         with arc.Context(w, digest=1, stream=stream.cuda_stream, **extra) as cxd:
+            if shard:
+                cxd.set_sources(my_sources)
             cxd.trace(0)
             sd = cxd.stats()
             seg_per_record = sd["segments"] / max(1, sd["deposit_records"])
@@ -268,6 +282,8 @@ def run_cuda(args):
     pin = [torch.from_numpy(np.ascontiguousarray(np.asarray(a, dtype=fdt))).pin_memory() for a in w.fields()]
     rates_host = [torch.empty(nc, dtype=torch.float64).pin_memory() for _ in range(4)]   # Gamma_HI, Gamma_HeI, Gamma_HeII, heat_total
     cx2 = arc.Context(w, fields=[p.numpy() for p in pin], stream=stream.cuda_stream, **extra)
+    if shard:
+        cx2.set_sources(my_sources)
     h2d = 5 * nc * pin[0].element_size()
     d2h = 4 * nc * pin[0].element_size() + 4 * nc * 8
     e2e_seg = 0
@@ -275,7 +291,11 @@ def run_cuda(args):
     def e2e_step(i):
         hp = [p.numpy() for p in pin]
         arc.arc_set_fields(cx2.ctx, *hp)                                   # H2D: the five fields
-        arc.arc_trace(cx2.ctx, i)
+        if shard:
+            with torch.cuda.stream(stream):
+                sharded.trace_sharded(cx2, None, i)
+        else:
+            arc.arc_trace(cx2.ctx, i)
         arc.arc_update_chemistry(cx2.ctx, w.dt_s)
         arc.arc_get_fields(cx2.ctx, None, hp[1], hp[2], hp[3], hp[4])      # D2H: the four updated fields
         rh = [r.numpy() for r in rates_host]
@@ -305,9 +325,10 @@ def run_cuda(args):
         achieved = bytes_seg * tot_seg / (kms * 1e-3) / 1e9 if kms > 0 else 0.0
         line = {
             "metric": METRIC, "value": job_throughput(seg_all, dev_ms_max), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True, "scaling": "strong" if shard else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, paper_1807_07094_b200/workloads.py)",
-            "config": dict(describe(w), parallelism="replicas" if world > 1 else "single-gpu",
+            "config": dict(describe(w), parallelism=(f"sources sharded over {world} rank(s), one all-reduce of the accumulators per step" if shard
+                                                     else ("replicas" if world > 1 else "single-gpu")),
                            l2_policy="inputs larger than L2" if (nc * nb * (bytes_seg // nb)) > 126e6 else "working set fits L2 (small config)",
                            trace_grid_blocks=trace_grid, deposit=args.deposit, geom_corr=args.geom_corr, thin_tau=args.thin_tau),
             "e2e": {"value": job_throughput(e2e_seg_all, e2e_ms_max), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
@@ -356,6 +377,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--geom-corr", type=int, default=0, help="arc_params.geom_corr (PAPER.md:100-114): 0 none (the north_star path), 1 f_c, 2 f_c + secondary, 3 f_c^2")
     ap.add_argument("--thin-tau", type=float, default=0.0, help="arc_params.thin_tau (PAPER.md:116-130): 0 off (the north_star path), 0.1 in the paper")
+    ap.add_argument("--shard", default="none", choices=["none", "sources"],
+                    help="N > 1: 'none' = independent replicas (the north_star path, weak scaling); 'sources' = the sources divided among the "
+                         "ranks, one all-reduce of the accumulators per step (paper_1807_07094_b200/sharded.py; strong scaling)")
     ap.add_argument("--sources", type=int, default=0, help="profiling aid: keep only the first K sources of the workload")
     ap.add_argument("--deposit", type=int, default=0, help="arc_params.deposit: 0 auto, 1 per-lane REDs, 2 warp-aggregated")
     args = ap.parse_args()

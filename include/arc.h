@@ -158,6 +158,24 @@ int arc_trace(arc_ctx *c, int step, arc_rates *out);
 int arc_get_rates(arc_ctx *c, double *Gamma_HI, double *Gamma_HeI, double *Gamma_HeII,
                   double *heat_HI, double *heat_HeI, double *heat_HeII, double *heat_total, int where);
 
+/* Source-sharded tracing ("the total ionization rate ... is the sum of the contributions of all
+ * sources", :134, :231): the absorbed-photon accumulators are linear in the sources, so several contexts (one per GPU,
+ * same fields, each with its own share of the sources) can trace independently and add their accumulators before the
+ * rates are formed.
+ *   arc_trace_partial : rows a1-a9 of a trace for THIS context's sources (zero, opacity table, rays); no rates yet -
+ *                       arc_get_rates / arc_update_chemistry return ARC_ESTATE until arc_finalize.  Errors as arc_trace.
+ *   arc_accum_device  : library-owned DEVICE pointer to the accumulators and their length in doubles
+ *                       (N^3 records of nbins doubles, padded to an even count when nbins > 1; padding stays 0), for an
+ *                       in-place element-wise sum over the shards by the caller (e.g. ncclAllReduce on the context's
+ *                       stream).  Valid until arc_destroy; contents defined between arc_trace_partial and arc_finalize.
+ *   arc_finalize      : row a10 (rates from whatever the accumulators now hold).  out may be NULL.  ARC_ESTATE without
+ *                       a pending arc_trace_partial (setting fields, sources, spectrum or parameters discards it).
+ * Statistics (arc_get_stats) stay per context: segments, rays, emitted, escaped are this shard's; `absorbed` is the sum
+ * over cells of the accumulators at arc_finalize, i.e. of all shards after the caller's sum. */
+int arc_trace_partial(arc_ctx *c, int step);
+int arc_accum_device(arc_ctx *c, double **A, int64_t *n_doubles);
+int arc_finalize(arc_ctx *c, arc_rates *out);
+
 /* Raw accumulators of the last trace: absorbed photons/s, layout [cell][bin], N^3*nbins doubles. */
 int arc_get_accum(arc_ctx *c, double *A, int where);
 

@@ -29,6 +29,7 @@ LIB_PATH = os.path.join(_HERE, "libarc_b200.so")
 
 EXPORTS = ["arc_create_grid", "arc_destroy", "arc_default_params", "arc_set_params", "arc_set_stream",
            "arc_set_fields", "arc_get_fields", "arc_set_spectrum", "arc_set_sources", "arc_set_emission_mask", "arc_get_thin_radii", "arc_set_thin_radii", "arc_trace",
+           "arc_trace_partial", "arc_accum_device", "arc_finalize",
            "arc_get_rates", "arc_get_accum", "arc_update_chemistry", "arc_suggest_dt", "arc_synchronize", "arc_get_stats",
            "arc_trace_debug", "arc_pix2vec", "arc_last_error", "arc_version"]
 
@@ -92,6 +93,9 @@ def lib():
         l.arc_set_sources.argtypes = [vp, i32] + [vp] * 3
         l.arc_trace.argtypes = [vp, i32, C.POINTER(arc_rates)]
         l.arc_get_rates.argtypes = [vp] + [vp] * 7 + [i32]
+        l.arc_trace_partial.argtypes = [vp, i32]
+        l.arc_accum_device.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_int64)]
+        l.arc_finalize.argtypes = [vp, C.POINTER(arc_rates)]
         l.arc_get_accum.argtypes = [vp, vp, i32]
         l.arc_update_chemistry.argtypes = [vp, dbl]
         l.arc_suggest_dt.argtypes = [vp, i32, dbl, vp, vp]
@@ -205,6 +209,26 @@ def arc_trace(ctx, step: int = 0) -> arc_rates:
     """-> arc_rates: library-owned DEVICE pointers, valid until the next arc_trace / arc_destroy."""
     out = arc_rates()
     _check(ctx, lib().arc_trace(ctx, int(step), C.byref(out)))
+    return out
+
+
+def arc_trace_partial(ctx, step: int = 0):
+    """rows a1-a9 for this context's sources only (source-sharded tracing); rates after arc_finalize"""
+    return _check(ctx, lib().arc_trace_partial(ctx, int(step)))
+
+
+def arc_accum_device(ctx):
+    """-> (device pointer, number of doubles) of the library-owned accumulators"""
+    p = C.c_void_p()
+    n = C.c_int64()
+    _check(ctx, lib().arc_accum_device(ctx, C.byref(p), C.byref(n)))
+    return int(p.value or 0), int(n.value)
+
+
+def arc_finalize(ctx) -> arc_rates:
+    """row a10 from whatever the accumulators hold (after the caller's sum over shards)"""
+    out = arc_rates()
+    _check(ctx, lib().arc_finalize(ctx, C.byref(out)))
     return out
 
 
@@ -352,6 +376,22 @@ class Context:
 
     def trace(self, step=0):
         return arc_trace(self.ctx, step)
+
+    def trace_partial(self, step=0):
+        return arc_trace_partial(self.ctx, step)
+
+    def finalize(self):
+        return arc_finalize(self.ctx)
+
+    def accum_tensor(self):
+        """the library's accumulators as a torch CUDA tensor that ALIASES them (no copy), for an in-place reduction"""
+        import torch
+        ptr, n = arc_accum_device(self.ctx)
+
+        class _Alias:                               # __cuda_array_interface__ v2: 1-d float64, C order
+            __cuda_array_interface__ = {"shape": (n,), "typestr": "<f8", "data": (ptr, False), "version": 2, "strides": None}
+
+        return torch.as_tensor(_Alias(), device="cuda")
 
     def rates(self):
         """-> Gamma[3, nc], heat[3, nc], heat_total[nc] as host arrays."""

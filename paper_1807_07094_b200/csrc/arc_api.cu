@@ -120,7 +120,7 @@ int arc_set_params(arc_ctx *c, const arc_params *p)
     if (p->geom_corr != ARC_GEOM_NONE && p->deposit != ARC_DEPOSIT_AUTO)
         return fail(c, ARC_EINVAL, "arc_set_params: the geometric correction is built for deposit = ARC_DEPOSIT_AUTO only");
     c->p = *p;
-    c->have_rates = false;
+    c->have_rates = false; c->have_accum = false;
     return ARC_OK;
 }
 
@@ -144,7 +144,7 @@ int arc_set_fields(arc_ctx *c, const void *n_H, const void *x_HI, const void *x_
         if (src[i]) CK(cudaMemcpyAsync(c->f[i], src[i], (size_t)c->ncell * esize(c), kind, c->stream));
     if (where == ARC_HOST) CK(cudaStreamSynchronize(c->stream));     // the caller may reuse pageable buffers
     c->have_fields = true;
-    c->have_rates = false;
+    c->have_rates = false; c->have_accum = false;
     return ARC_OK;
 }
 
@@ -183,7 +183,7 @@ int arc_set_spectrum(arc_ctx *c, int nbins, const double *E_eV, const double *si
         c->spec.E[v] = E_eV[v]; c->spec.sig[0][v] = sig_HI[v]; c->spec.sig[1][v] = sig_HeI[v]; c->spec.sig[2][v] = sig_HeII[v];
     }
     c->have_spec = true;
-    c->have_rates = false;
+    c->have_rates = false; c->have_accum = false;
     return ARC_OK;
 }
 
@@ -224,7 +224,7 @@ int arc_set_sources(arc_ctx *c, int nsrc, const double *pos_cm, const double *Nd
     }
     c->nsrc = nsrc;
     c->have_src = true;
-    c->have_rates = false;
+    c->have_rates = false; c->have_accum = false;
     return ARC_OK;
 }
 
@@ -245,7 +245,7 @@ int arc_set_thin_radii(arc_ctx *c, const double *R_cells)
     for (int s = 0; s < c->nsrc; ++s)
         if (!(R_cells[s] >= 0.0) || !std::isfinite(R_cells[s])) return fail(c, ARC_EINVAL, "arc_set_thin_radii: radii must be finite and >= 0");
     for (int s = 0; s < c->nsrc; ++s) c->h_R[(size_t)s] = R_cells[s];
-    c->have_rates = false;
+    c->have_rates = false; c->have_accum = false;
     return ARC_OK;
 }
 
@@ -260,7 +260,7 @@ int arc_set_emission_mask(arc_ctx *c, const uint8_t *blocked, int level)
     if (!blocked) {
         c->h_nopen.assign((size_t)c->nsrc, -1.0);
         for (int s = 0; s < c->nsrc; ++s) for (int v = 0; v < nb; ++v) c->emitted[v] += c->h_src_S[(size_t)s * nb + v];
-        c->have_rates = false;
+        c->have_rates = false; c->have_accum = false;
         return ARC_OK;
     }
     if (level != c->p.l0) return fail(c, ARC_EINVAL, "arc_set_emission_mask: level must equal arc_params.l0");
@@ -276,7 +276,7 @@ int arc_set_emission_mask(arc_ctx *c, const uint8_t *blocked, int level)
         CK(cudaMemcpy(c->d_blocked, blocked, (size_t)c->nsrc * npix0, cudaMemcpyHostToDevice));
     }
     c->mask_level = level;
-    c->have_rates = false;
+    c->have_rates = false; c->have_accum = false;
     return ARC_OK;
 }
 

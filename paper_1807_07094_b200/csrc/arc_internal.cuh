@@ -129,8 +129,10 @@ struct arc_ctx {
     unsigned long long *d_dt = 0;     // [2] arc_suggest_dt: min dt (bits of a positive double), cells used
     int n_sm = 0;
     int trace_grid = 0;
-    cudaEvent_t ev[8];                // 0..4: trace call (start, after opacity, after kernel, after finalize); 5,6: chemistry
+    cudaEvent_t ev[8];                // 0..3: trace call (start, after opacity, after kernel, after finalize); 4,7: arc_finalize; 5,6: chemistry
     bool traced_once = false, chem_once = false;
+    bool have_accum = false;          // arc_trace_partial ran: the accumulators wait for arc_finalize
+    bool finalize_split = false;      // the last finalise pass was arc_finalize's (events 4, 7)
     std::string err;
 };
 

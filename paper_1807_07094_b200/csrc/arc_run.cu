@@ -26,7 +26,7 @@ static int device_error(arc_ctx *c)
     SchedState h;
     CK(cudaMemcpy(&h, c->d_sched, sizeof(h), cudaMemcpyDeviceToHost));
     if (h.error == ARC_DEV_OK && h.in_flight == 0) return ARC_OK;
-    c->have_rates = false;
+    c->have_rates = false; c->have_accum = false;
     switch (h.error) {
         case ARC_DEV_STACK_OVERFLOW: return fail(c, ARC_EOVERFLOW, "arc_trace: a warp's work stack overflowed; rates are invalid");
         case ARC_DEV_LOG_OVERFLOW: return fail(c, ARC_EOVERFLOW, "arc_trace_debug: ray log too small");
@@ -36,7 +36,7 @@ static int device_error(arc_ctx *c)
     }
 }
 
-static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, unsigned int *d_seq, int *d_cell)
+static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, unsigned int *d_seq, int *d_cell, bool finalize = true)
 {
     if (!c->have_fields) return fail(c, ARC_ESTATE, "arc_trace: no fields set (arc_set_fields)");
     if (!c->have_spec) return fail(c, ARC_ESTATE, "arc_trace: no spectrum set (arc_set_spectrum)");
@@ -135,10 +135,12 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
     CK(cudaEventRecord(c->ev[1], c->stream));
     CK(arc_launch_trace(c, a, log != nullptr, nullptr));
     CK(cudaEventRecord(c->ev[2], c->stream));
-    CK(arc_launch_finalize(c));
+    if (finalize) CK(arc_launch_finalize(c));          // arc_trace_partial leaves a10 to arc_finalize
     CK(cudaEventRecord(c->ev[3], c->stream));
     c->traced_once = true;
-    c->have_rates = true;
+    c->have_rates = finalize;
+    c->have_accum = !finalize;
+    c->finalize_split = false;
     if (thin && c->nsrc > 0) {                 // (ii): the radii this trace found are the next trace's
         std::vector<unsigned long long> bits((size_t)c->nsrc);
         CK(cudaMemcpyAsync(bits.data(), c->d_Rnext, sizeof(unsigned long long) * c->nsrc, cudaMemcpyDeviceToHost, c->stream));
@@ -177,6 +179,37 @@ int arc_trace(arc_ctx *c, int step, arc_rates *out)
     const int rc = run_trace(c, nullptr, nullptr, nullptr, nullptr);
     if (rc == ARC_OK && out) fill_rates(c, out);
     return rc;
+}
+
+int arc_trace_partial(arc_ctx *c, int step)
+{
+    (void)step;
+    if (!c) return ARC_EINVAL;
+    return run_trace(c, nullptr, nullptr, nullptr, nullptr, false);
+}
+
+int arc_accum_device(arc_ctx *c, double **A, int64_t *n_doubles)
+{
+    if (!c || !A || !n_doubles) return ARC_EINVAL;
+    if (!c->have_spec) return fail(c, ARC_ESTATE, "arc_accum_device: no spectrum set (the record length is the bin count)");
+    *A = c->d_A;
+    *n_doubles = (int64_t)c->ncell * arc_nbp(c->spec.nb);
+    return ARC_OK;
+}
+
+int arc_finalize(arc_ctx *c, arc_rates *out)
+{
+    if (!c) return ARC_EINVAL;
+    if (!c->have_accum) return fail(c, ARC_ESTATE, "arc_finalize: no partial trace to finalise (call arc_trace_partial; setting fields, sources, spectrum or parameters discards it)");
+    CK(cudaEventRecord(c->ev[4], c->stream));
+    CK(arc_launch_finalize(c));
+    CK(cudaEventRecord(c->ev[7], c->stream));
+    c->have_accum = false;
+    c->have_rates = true;
+    c->finalize_split = true;
+    if (!c->p.async) CK(cudaStreamSynchronize(c->stream));
+    if (out) fill_rates(c, out);
+    return ARC_OK;
 }
 
 int arc_trace_debug(arc_ctx *c, int step, arc_raylog *log)
@@ -226,7 +259,7 @@ int arc_get_accum(arc_ctx *c, double *A, int where)
 {
     if (!c || !A) return ARC_EINVAL;
     if (where != ARC_HOST && where != ARC_DEVICE) return fail(c, ARC_EINVAL, "arc_get_accum: bad `where`");
-    if (!c->have_rates) return fail(c, ARC_ESTATE, "arc_get_accum: no valid trace (call arc_trace)");
+    if (!c->have_rates && !c->have_accum) return fail(c, ARC_ESTATE, "arc_get_accum: no valid trace (call arc_trace)");
     const cudaMemcpyKind kind = (where == ARC_HOST) ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
     const int nb = c->spec.nb, nbp = arc_nbp(nb);        // device rows are padded to nbp doubles; the caller gets [cell][nb]
     if (nbp == nb) CK(cudaMemcpyAsync(A, c->d_A, (size_t)c->ncell * nb * sizeof(double), kind, c->stream));
@@ -299,6 +332,10 @@ int arc_get_stats(arc_ctx *c, arc_stats *s)
         cudaEventElapsedTime(&s->opacity_ms, c->ev[0], c->ev[1]);
         cudaEventElapsedTime(&s->trace_kernel_ms, c->ev[1], c->ev[2]);
         cudaEventElapsedTime(&s->finalize_ms, c->ev[2], c->ev[3]);
+        if (c->finalize_split) {                  // arc_trace_partial + arc_finalize: the finalise pass was timed on its own
+            cudaEventElapsedTime(&s->finalize_ms, c->ev[4], c->ev[7]);
+            s->trace_ms += s->finalize_ms;
+        }
     }
     if (c->chem_once) cudaEventElapsedTime(&s->chem_ms, c->ev[5], c->ev[6]);
     cudaGetLastError();
