@@ -18,8 +18,10 @@
  * brute-force line sampling of cell sequences, exact attenuation on axis-aligned rays, photon
  * conservation to 1e-10, partition of unity of the species weights, BDF closed forms, the
  * analytic Stromgren radius/growth.
- * PARITY UNPINNED: rate-coefficient fits other than alpha_B(1e4 K) = 2.59e-13
- * and the cooling function (PAPER.md:162,172 cite Hui & Gnedin 1997; Fig. 2 is an image only).
+ * Rate table (PAPER.md:162,172 cite Hui & Gnedin 1997; Fig. 2 is an image only): alpha_B(1e4 K) = 2.59e-13 is
+ * the paper's; the recombination coefficients and the recombination cooling are pinned against the
+ * standard tabulated values (tests/golden/textbook_rates.txt), He III by the hydrogenic scaling.
+ * PARITY UNPINNED: the collisional-ionisation, collisional-excitation, dielectronic and free-free fits.
  *
  * Build: gcc -O2 -ffp-contract=off -fno-fast-math -shared -fPIC arc_oracle.c -lm
  */

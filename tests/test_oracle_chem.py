@@ -1,6 +1,7 @@
 """Pins for the oracle's chemistry/thermal update (O6) and for trace+chemistry together
 (the analytic Stromgren sphere)."""
 import math
+import os
 
 import numpy as np
 import pytest
@@ -158,3 +159,40 @@ def test_stromgren_coarse_steps_reaches_the_papers_accuracy():
     assert ratios[0] < 0.5                                       # the fixed-step lag the paper describes
     assert abs(ratios[-1] - 1) < float(GOLD["stromgren_accuracy"])
     assert abs(radii[-1] / R_S / (1 - math.exp(-5)) ** (1 / 3) - 1) < 0.05
+
+
+def _textbook():
+    rows = []
+    with open(os.path.join(os.path.dirname(__file__), "golden", "textbook_rates.txt")) as f:
+        for line in f:
+            line = line.split("#")[0].split()
+            if len(line) == 4:
+                rows.append((line[0], float(line[1]), float(line[2]), float(line[3])))
+    return rows
+
+
+def test_recombination_coefficients_and_cooling_match_the_textbook_tables():
+    """Reading G11: the fits typed into the oracle against the standard tabulated recombination coefficients
+    (tests/golden/textbook_rates.txt) - a wrong exponent, prefactor or threshold temperature moves them by far more
+    than the tolerance.  Collisional ionisation / excitation stay unpinned."""
+    KB = 1.380649e-16
+    rows = _textbook()
+    assert len(rows) == 10
+    for key, T, val, tol in rows:
+        caseB = 1 if "_B_" in key else 0
+        o = orc.rate_coeffs(T, caseB=caseB, coll_ion=1)
+        got = {"alpha_A_HII": o[0], "alpha_B_HII": o[0], "alpha_A_HeII": o[1], "alpha_B_HeII": o[1],
+               "beta_A_HII": o[6] / (KB * T), "beta_B_HII": o[6] / (KB * T)}[key]
+        assert abs(got / val - 1.0) <= tol, (key, T, got, val)
+
+
+def test_helium_iii_follows_the_hydrogenic_scaling():
+    """alpha(Z, T) = Z alpha_H(T / Z^2) for a hydrogenic ion: He III at 4 T equals 2 x H II at T (to the ratio of the
+    threshold temperatures, 631515 / 157807 = 4.0018), and the recombination cooling k_B T beta scales by Z^3 = 8 in
+    beta's units, i.e. 8 x 4 in erg cm^3 / s at 4 T."""
+    for caseB in (0, 1):
+        for T in (5e3, 1e4, 5e4):
+            h = orc.rate_coeffs(T, caseB=caseB)
+            he = orc.rate_coeffs(4.0 * T, caseB=caseB)
+            assert abs(he[2] / (2.0 * h[0]) - 1.0) < 2e-3
+            assert abs(he[8] / (32.0 * h[6]) - 1.0) < 2e-3
