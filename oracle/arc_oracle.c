@@ -20,8 +20,9 @@
  * analytic Stromgren radius/growth.
  * Rate table (PAPER.md:162,172 cite Hui & Gnedin 1997; Fig. 2 is an image only): alpha_B(1e4 K) = 2.59e-13 is
  * the paper's; the recombination coefficients and the recombination cooling are pinned against the
- * standard tabulated values (tests/golden/textbook_rates.txt), He III by the hydrogenic scaling.
- * PARITY UNPINNED: the collisional-ionisation, collisional-excitation, dielectronic and free-free fits.
+ * standard tabulated values (tests/golden/textbook_rates.txt), He III by the hydrogenic scaling, collisional
+ * ionisation against Voronov's (1997) independent fit (within 25 %).
+ * PARITY UNPINNED: the collisional-excitation, dielectronic and free-free fits.
  *
  * Build: gcc -O2 -ffp-contract=off -fno-fast-math -shared -fPIC arc_oracle.c -lm
  */

@@ -164,8 +164,8 @@ __device__ __forceinline__ void chem_load(Cell &c, long long i, long long ncell,
     c.t = 0.0; c.n = 0;
 }
 
-// Isothermal runs (configs 1-2): the rate table is evaluated once per cell and a sub-cycle is a few dozen flops, so
-// one thread keeps one cell; fully coalesced grid-stride pass.
+// Isothermal runs (configs 1-2): the rate table does not change during the call and a sub-cycle is a few dozen flops,
+// so one thread keeps one cell; fully coalesced grid-stride pass.
 template <typename FT>
 __global__ void __launch_bounds__(128) arc_chem_iso_kernel(long long ncell, double dt, double Yp, double eps, double x_floor,
                                                           int max_sub, ChemK q,
@@ -174,10 +174,24 @@ __global__ void __launch_bounds__(128) arc_chem_iso_kernel(long long ncell, doub
                                                           const double *__restrict__ rates, DevStats *stats)
 {
     unsigned long long my_sub = 0; unsigned int my_max = 0;
+    // an isothermal box usually has ONE temperature: the table at the block's first cell is evaluated once (first warp)
+    // and shared; a cell at another temperature evaluates its own (same function, same argument: same bits)
+    __shared__ Coef s_k;
+    __shared__ double s_T;
+    {
+        const long long first = blockIdx.x * (long long)blockDim.x;
+        if (threadIdx.x < 32) {
+            Coef k0;
+            const double T0 = (double)Tf[first < ncell ? first : 0];
+            rate_table(T0, q, k0);
+            if (threadIdx.x == 0) { s_k = k0; s_T = T0; }
+        }
+        __syncthreads();
+    }
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < ncell; i += (long long)gridDim.x * blockDim.x) {
         Cell c; Coef k;
         chem_load<FT, true>(c, i, ncell, Yp, nHf, xHIf, xHeIf, xHeIIf, Tf, rates);
-        rate_table(c.T, q, k);
+        if (c.T == s_T) k = s_k; else rate_table(c.T, q, k);
         while (c.t < dt && c.n < max_sub) chem_subcycle<true>(c, k, q, dt, eps, x_floor, max_sub);
         xHIf[i] = (FT)c.x0; xHeIf[i] = (FT)c.x1; xHeIIf[i] = (FT)c.x2;
         my_sub += (unsigned long long)c.n;

@@ -186,6 +186,30 @@ def test_recombination_coefficients_and_cooling_match_the_textbook_tables():
         assert abs(got / val - 1.0) <= tol, (key, T, got, val)
 
 
+def test_collisional_ionisation_agrees_with_an_independent_published_fit():
+    """Reading G11: the Hui & Gnedin (1997) collisional-ionisation fits typed into the oracle against Voronov's (1997)
+    fit to the measured cross-sections (parameters in tests/golden/textbook_rates.txt), 2e4-1e6 K.  A wrong prefactor,
+    exponent or threshold moves the rate by factors, the two fits differ by < 25 %."""
+    pars = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "textbook_rates.txt")) as f:
+        for line in f:
+            t = line.split("#")[0].split()
+            if len(t) == 7 and t[0].startswith("voronov_"):
+                pars[t[0][8:]] = tuple(float(x) for x in t[1:])
+    assert sorted(pars) == ["HI", "HeI", "HeII"]
+    k_eV = 8.617333262e-5
+    for T in (2e4, 5e4, 1e5, 3e5, 1e6):
+        o = orc.rate_coeffs(T, caseB=1, coll_ion=1)
+        for j, sp in enumerate(("HI", "HeI", "HeII")):
+            dE, P, A, X, K, tol = pars[sp]
+            U = dE / (k_eV * T)
+            v = A * (1.0 + P * math.sqrt(U)) * U ** K * math.exp(-U) / (X + U)
+            assert abs(o[3 + j] / v - 1.0) < tol, (sp, T, o[3 + j], v)
+            assert abs(o[9 + j] / (o[3 + j] * dE * 1.602176634e-12) - 1.0) < 5e-3     # its cooling = threshold energy x rate
+    off = orc.rate_coeffs(1e5, caseB=1, coll_ion=0)
+    assert off[3] == off[4] == off[5] == 0.0 and off[9] == off[10] == off[11] == 0.0
+
+
 def test_helium_iii_follows_the_hydrogenic_scaling():
     """alpha(Z, T) = Z alpha_H(T / Z^2) for a hydrogenic ion: He III at 4 T equals 2 x H II at T (to the ratio of the
     threshold temperatures, 631515 / 157807 = 4.0018), and the recombination cooling k_B T beta scales by Z^3 = 8 in
