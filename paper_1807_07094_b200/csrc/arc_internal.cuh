@@ -32,15 +32,22 @@ struct __align__(16) FamRec {
     double P[NB];
 };
 
+// Every word that idle warps poll or working warps update sits in its own 256-byte block: thousands of idle warps polling
+// ONE line keep a single L2 slice saturated (measured: with 3 blocks per SM a lone ray tree ran 2x slower than with 1),
+// and the working warps' own scheduler accesses queue up behind the polls.  Spread out, the words hash to different slices.
+#ifndef ARC_SCHED_ALIGN
+#define ARC_SCHED_ALIGN 256
+#endif
 struct SchedState {
-    long long in_flight;                 // families alive anywhere, as known through flushes
-    unsigned long long seed_next;        // next unclaimed root family
-    unsigned long long q_head, q_tail;   // donation queue tickets (reserved pops / pushes)
-    long long q_count;                   // counting semaphore: published - claimed entries (may dip below 0)
-    int hungry;                          // warps idling for work
-    int error;                           // ARC_DEV_*
-    unsigned long long q_high;           // max(q_tail - q_head) seen
-    unsigned long long log_n;            // ray-log entries written
+    alignas(ARC_SCHED_ALIGN) long long in_flight;            // families alive anywhere, as known through flushes
+    alignas(ARC_SCHED_ALIGN) unsigned long long seed_next;   // next unclaimed root family
+    alignas(ARC_SCHED_ALIGN) unsigned long long q_head;      // donation queue tickets: reserved pops
+    alignas(ARC_SCHED_ALIGN) unsigned long long q_tail;      // ... and pushes
+    alignas(ARC_SCHED_ALIGN) long long q_count;              // counting semaphore: published - claimed entries (may dip below 0)
+    alignas(ARC_SCHED_ALIGN) int hungry;                     // warps idling for work
+    alignas(ARC_SCHED_ALIGN) int error;                      // ARC_DEV_*
+    alignas(ARC_SCHED_ALIGN) unsigned long long q_high;      // max(q_tail - q_head) seen
+    unsigned long long log_n;                                // ray-log entries written
 };
 
 struct DevStats {
