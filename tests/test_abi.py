@@ -39,6 +39,7 @@ def test_every_declared_entry_point_is_exported_and_bound(lib):
 
 def test_library_links_only_the_cuda_runtime(lib):
     out = subprocess.run(["ldd", arc.LIB_PATH], capture_output=True, text=True).stdout
+    out = re.sub(r"\(0x[0-9a-f]+\)", "", out)             # load addresses are random hex: "c10" may turn up in one
     for forbidden in ("torch", "python", "oracle", "c10", "cublas", "nccl"):
         assert forbidden not in out.lower(), out
 
