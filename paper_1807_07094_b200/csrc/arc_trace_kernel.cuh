@@ -29,6 +29,12 @@
 #define FLAG_LOG 1          // template flag: per-ray logging (arc_trace_debug)
 #define FLAG_DIGEST 2       // template flag: accumulate the order-independent traversal digest
 #define FLAG_GEOM 4         // template flag: geometric correction of the deposit (Eq. 2-3), mode in TraceArgs::geom
+#ifndef ARC_GREEDY_MIN_INFLIGHT
+#define ARC_GREEDY_MIN_INFLIGHT 2048   // families alive above which idle warps take whole batches from the donation queue
+#endif
+#ifndef ARC_POOL_PER_HUNGRY
+#define ARC_POOL_PER_HUNGRY ARC_BATCH_FAM      // donors keep the pool at this many families per idle warp
+#endif
 #define FLAG_THIN 8         // template flag: track, per source, the radius up to which tau (bin 0) stays below thin_tau
 
 #ifndef ARC_TRACE_MIN_BLOCKS
@@ -260,8 +266,16 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                 if (lane == 0) {
                     const long long avail = ld_volatile_s64(&sc->q_count);
                     if (avail > 0) {
-                        const int hungry_now = max(ld_volatile_s32(&sc->hungry), 1);
-                        const long long want = max(1ll, min((long long)ARC_BATCH_FAM, avail / hungry_now));
+                        // How much to take.  An SM's issue slots are used up by ~8 warps, so once a trace has deep levels alive
+                        // (many families in flight: long rays) few FULL warps beat many warps with 4 of 32 lanes busy: take a
+                        // whole batch.  While few families exist (start of a trace, tiny traces: short rays, the queue hop is
+                        // what costs) an equal share per idle warp spreads the tree fastest.  Measured, DESIGN.md 6.2.
+                        long long want;
+                        if (ld_volatile_s64(&sc->in_flight) >= ARC_GREEDY_MIN_INFLIGHT) want = min((long long)ARC_BATCH_FAM, avail);
+                        else {
+                            const int hungry_now = max(ld_volatile_s32(&sc->hungry), 1);
+                            want = max(1ll, min((long long)ARC_BATCH_FAM, avail / hungry_now));
+                        }
                         const long long before = (long long)atomicAdd((unsigned long long *)&sc->q_count, (unsigned long long)(-want));
                         const long long got = max(0ll, min(before, want));
                         if (got < want) atomicAdd((unsigned long long *)&sc->q_count, (unsigned long long)(want - got));
@@ -750,7 +764,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                 // approximate (plain loads), the ring is sized so that every warp overshooting at once still fits
                 const unsigned long long t = ld_volatile_u64(&sc->q_tail), hq = ld_volatile_u64(&sc->q_head);
                 const unsigned long long level_now = t > hq ? t - hq : 0ull;
-                if (level_now >= (unsigned long long)min(hungry * 4, ARC_QUEUE_LOW)) nd = 0;
+                if (level_now >= (unsigned long long)min(hungry * ARC_POOL_PER_HUNGRY, ARC_QUEUE_LOW)) nd = 0;
                 else {
                     // flush first: donated families must be covered by the global counter before they are visible
                     if (delta != 0) atomicAdd((unsigned long long *)&sc->in_flight, (unsigned long long)delta);
