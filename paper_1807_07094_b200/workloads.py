@@ -238,7 +238,7 @@ def _peaks_workload(name, N, nsrc, sigma_ln, seed, n_steps, kmax=None, state="ne
     else:
         x_HI = np.full(n, 1.0 - 1.2e-3, dtp); x_HeI = np.full(n, 1.0 - 1.2e-3, dtp)
         x_HeII = np.full(n, 1.2e-3, dtp); T = np.full(n, 100.0, dtp)
-    return Workload(name, N, box, "f32", n3.ravel().astype(dtp), x_HI, x_HeI, x_HeII, T,
+    return Workload(name + ("_T" if state == "transparent" else ""), N, box, "f32", n3.ravel().astype(dtp), x_HI, x_HeI, x_HeII, T,
                     E, s1, s2, s3, _cell_centre_cm(pk, N, box), Ndot, np.tile(frac, (nsrc, 1)),
                     0.05 * n_atoms / Ndot.sum(), n_steps, p)
 
