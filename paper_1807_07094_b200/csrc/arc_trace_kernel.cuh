@@ -15,7 +15,8 @@
 //  * Each warp owns a LIFO stack in global memory (depth-first => bounded memory: <= 32 families per
 //    level).  Survivors of a batch are compacted with a ballot/popc prefix and pushed in one step.
 //  * Load balance: root families come from a global seed counter; idle warps raise `hungry` and busy
-//    warps donate the shallow half of their stack (biggest subtrees) through a bounded MPMC ticket queue.
+//    warps keep their next batch and donate the rest of their stack, shallow end first (biggest subtrees),
+//    through a bounded MPMC ticket queue; idle warps take whole batches once the trace is deep.
 //  * Deposit: fire-and-forget fp64 REDs into the cell's accumulator record.  The RED path costs
 //    per LANE (one L1 wavefront / L2 sector op each), so lanes of a warp that are in the same cell in the same
 //    iteration - siblings and neighbouring pixels run almost parallel less than a cell apart - are first summed
@@ -31,6 +32,9 @@
 #define FLAG_GEOM 4         // template flag: geometric correction of the deposit (Eq. 2-3), mode in TraceArgs::geom
 #ifndef ARC_GREEDY_MIN_INFLIGHT
 #define ARC_GREEDY_MIN_INFLIGHT 2048   // families alive above which idle warps take whole batches from the donation queue
+#endif
+#ifndef ARC_DONATE_KEEP
+#define ARC_DONATE_KEEP 8              // a donor keeps its next batch (8 families) and gives away the rest, 32 at a time (0: gives half its ring)
 #endif
 #ifndef ARC_POOL_PER_HUNGRY
 #define ARC_POOL_PER_HUNGRY ARC_BATCH_FAM      // donors keep the pool at this many families per idle warp
@@ -750,14 +754,19 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
         }
         __syncwarp();
 
-        // ------------------------------------------------------------------ donate the shallow half if someone is idle
+        // ------------------------------------------------------------------ donate the shallow end of the ring if someone is idle
         int hungry = 0, err = 0;
         if (lane == 0) { hungry = ld_volatile_s32(&sc->hungry); err = ld_volatile_s32(&sc->error); }
         hungry = __shfl_sync(0xffffffffu, hungry, 0);
         err = __shfl_sync(0xffffffffu, err, 0);
         if (err) quit = true;
-        if (!quit && hungry > 0 && top - bot >= 2) {
-            int nd = (int)min((top - bot) / 2, 32u);
+#if ARC_DONATE_KEEP > 0
+        const unsigned nd_max = min(top - bot > (unsigned)ARC_DONATE_KEEP ? top - bot - (unsigned)ARC_DONATE_KEEP : 0u, 32u);   // keep the next batch(es), give the rest
+#else
+        const unsigned nd_max = min((top - bot) / 2, 32u);
+#endif
+        if (!quit && hungry > 0 && nd_max > 0) {
+            int nd = (int)nd_max;
             unsigned long long ticket = 0;
             if (lane == 0) {
                 // donate only while the pool is short of what the idle warps can take; the level test is
