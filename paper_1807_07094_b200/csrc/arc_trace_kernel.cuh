@@ -270,9 +270,9 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                 if (lane == 0) {
                     const long long avail = ld_volatile_s64(&sc->q_count);
                     if (avail > 0) {
-                        // How much to take.  An SM's issue slots are used up by ~8 warps, so once a trace has deep levels alive
-                        // (many families in flight: long rays) few FULL warps beat many warps with 4 of 32 lanes busy: take a
-                        // whole batch.  While few families exist (start of a trace, tiny traces: short rays, the queue hop is
+                        // How much to take.  A warp iteration costs the same with 4 lanes busy as with 32, so once a trace has
+                        // deep levels alive (many families in flight: long rays) a whole batch per warp beats one family per
+                        // idle warp.  While few families exist (start of a trace, tiny traces: short rays, the queue hop is
                         // what costs) an equal share per idle warp spreads the tree fastest.  Measured, DESIGN.md 6.2.
                         long long want;
                         if (ld_volatile_s64(&sc->in_flight) >= ARC_GREEDY_MIN_INFLIGHT) want = min((long long)ARC_BATCH_FAM, avail);
