@@ -21,8 +21,16 @@
  * Rate table (PAPER.md:162,172 cite Hui & Gnedin 1997; Fig. 2 is an image only): alpha_B(1e4 K) = 2.59e-13 is
  * the paper's; the recombination coefficients and the recombination cooling are pinned against the
  * standard tabulated values (tests/golden/textbook_rates.txt), He III by the hydrogenic scaling, collisional
- * ionisation against Voronov's (1997) independent fit (within 25 %).
- * PARITY UNPINNED: the collisional-excitation, dielectronic and free-free fits.
+ * ionisation against Voronov's (1997) independent fit (within 25 %), collisional-excitation cooling by its Lyman-alpha
+ * thresholds (3/4 of the ionisation energies) and against the textbook collision strengths (25 % for H I, a factor two
+ * for He II - the classic fit is no better than that), free-free against the textbook emissivity and Gaunt-factor
+ * range, dielectronic recombination against the published fit parameters and the 40.8 eV core excitation.
+ * Chemistry (tests/test_oracle_chem_pins.py): n_e against PAPER.md:73 in n_b, A_H, A_He; every term of the H I / He I /
+ * He II backward differences (one-step identity + conservation of helium nuclei + closed-form equilibrium and cascade);
+ * the energy update, T(E) and the sub-cycle limiter (one-step identities in states that isolate each cooling process,
+ * mu by hand, convergence to scipy's integration of Eq. 4 + the energy equation, thermal-equilibrium root).
+ * PARITY UNPINNED: nothing by structure; by VALUE the textbook numbers in tests/golden/textbook_rates.txt were typed
+ * from outside this container (labelled there), and the He II excitation magnitude is only pinned to a factor two.
  *
  * Build: gcc -O2 -ffp-contract=off -fno-fast-math -shared -fPIC arc_oracle.c -lm
  */
