@@ -13,7 +13,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "arc_oracle.c")
-_LIB = os.path.join(_HERE, "libarc_oracle.so")
+# ARC_ORACLE_SANITIZE=1: the same source built with -fsanitize=address,undefined into a library of its own (run the
+# oracle's pin tests under it with LD_PRELOAD=$(gcc -print-file-name=libasan.so); profiles/r02_sanitizers.md)
+_SAN = os.environ.get("ARC_ORACLE_SANITIZE", "") not in ("", "0")
+_LIB = os.path.join(_HERE, "libarc_oracle_san.so" if _SAN else "libarc_oracle.so")
 
 MAXNB, MAXLEVEL = 8, 16
 END_SPLIT, END_DEPLETED, END_ESCAPED = 0, 1, 2
@@ -22,8 +25,9 @@ END_SPLIT, END_DEPLETED, END_ESCAPED = 0, 1, 2
 def build(force: bool = False) -> str:
     """gcc -O2, no FMA contraction, no fast-math (arithmetic contract C0)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        san = ["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] if _SAN else []
         subprocess.check_call(["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-shared",
-                               "-fPIC", "-o", _LIB, _SRC, "-lm"])
+                               "-fPIC"] + san + ["-o", _LIB, _SRC, "-lm"])
     return _LIB
 
 

@@ -156,6 +156,20 @@ def test_small_persistent_grid_still_exact():
     assert_close(A, Ao, RTOL["f64"], "A")
 
 
+def test_four_bin_f32_three_blocks_donation_through_the_queue():
+    """the benched kernel variant's shape (4 bins, fp32 fields, transposed deposit) on a grid of 3 blocks: 24 warps share
+    40 sources, so most of the work travels through the donation queue.  Also the target of the compute-sanitizer runs
+    (profiles/r02_sanitizers.md)."""
+    w = wl.tiny(N=20, nsrc=40, nb=4, seed=33, dtype="f32", l0=1, kappa_scale=30.0)
+    (A, st, _), (Ao, so, _) = _trace_both(w, trace_blocks=3)
+    compare_trace_stats(st, so, 4, RTOL["f32"])
+    assert_close(A, Ao, RTOL["f32"], "A")
+    assert st["queue_high_water"] > 0 and st["ends"][1] > 0        # the queue was used; some rays ended DEPLETED
+    A0, st0, _ = run_gpu_trace(w, trace_blocks=3, digest=0)         # the timed variant (no digest): same integers, same sums
+    assert st0["segments"] == so["segments"] and np.array_equal(st0["ends"], so["ends"])
+    assert_close(A0, Ao, RTOL["f32"], "A (digest off)")
+
+
 def test_trace_is_repeatable_in_its_integers():
     w = wl.tiny(N=16, nsrc=4, nb=3, seed=41, dtype="f32", kappa_scale=10.0)
     with arc.Context(w, digest=1) as cx:
