@@ -19,7 +19,12 @@
  *  - work is enqueued on the stream given to arc_set_stream() (default: the legacy default stream).
  *    With arc_params.async == 0 (default) arc_trace()/arc_update_chemistry() synchronise that
  *    stream before returning and report device-side errors (e.g. ARC_EOVERFLOW) themselves; with
- *    async == 1 they only enqueue, and deferred errors surface from arc_synchronize()/arc_get_stats().
+ *    async == 1 they only enqueue.  A trace that failed on the device (ARC_EOVERFLOW, ARC_ECUDA) then leaves a sticky
+ *    device error: the kernels of every later call on that context (finalize, chemistry, time step, further traces) see
+ *    it and do NOTHING - fields and rates are never updated from an aborted trace - and the error is returned by the
+ *    first call that synchronises: arc_synchronize(), arc_get_stats(), arc_suggest_dt(), and arc_get_fields() /
+ *    arc_get_rates() / arc_get_accum() with ARC_HOST pointers.  Reporting it clears it (rates are then invalid:
+ *    ARC_ESTATE until the next arc_trace).  Device-pointer read-backs do not synchronise and cannot report.
  */
 #ifndef ARC_B200_H
 #define ARC_B200_H
@@ -70,7 +75,9 @@ typedef struct arc_params {
     int32_t trace_blocks;   /* persistent-kernel grid size; 0 = SM count x resident blocks per SM    */
     int32_t deposit;        /* how segments reach the accumulators: ARC_DEPOSIT_AUTO | _RED | _AGG | _QUAD        */
     int32_t geom_corr;      /* ARC_GEOM_NONE | _FC | _FC_SECONDARY | _FC2; needs deposit = AUTO */
-    int32_t reserved0;      /* keep 0                                                                 */
+    int32_t debug_fault;    /* test hook, keep 0: a non-zero ARC device error code (1 = work-stack overflow, 3 = watchdog,
+                               4 = runaway ray) makes every following trace start as if its kernel had raised it - the
+                               only way to exercise the error paths of async mode without breaking the tracer       */
     double  thin_tau;       /* optically thin inner region: 0 = off; > 0 (0.1 in the paper): every
                                arc_trace records, per source, the radius up to which tau of the first (softest) bin stays
                                below thin_tau on every ray, and the NEXT arc_trace gives the cells within that radius the
@@ -106,6 +113,8 @@ typedef struct arc_stats {
     int32_t  trace_grid;               /* thread blocks of the persistent kernel                          */
     int32_t  pad2;
     uint64_t deposit_records;          /* accumulator records sent to L2 (<= segments: warp-aggregated deposit) */
+    uint64_t kernel_launches;          /* kernels this context has launched since arc_create_grid (counted on the host at
+                                          every launch of the library's own kernels; memsets and copies are not kernels) */
 } arc_stats;
 
 /* Caller-provided HOST buffers for arc_trace_debug: one entry per segment (seq = 0,1,2,... within the
@@ -143,7 +152,8 @@ int arc_set_spectrum(arc_ctx *c, int nbins, const double *E_eV, const double *si
 
 /* Point sources: position [cm] in [0, box) on every axis (else ARC_EINVAL), photon
  * rate Ndot [1/s] and its split over the bins (rows of binfrac).  HOST pointers.  Call after
- * arc_set_spectrum (ARC_ESTATE otherwise). */
+ * arc_set_spectrum (ARC_ESTATE otherwise).  A position so close to the upper box face that pos/(box/N) rounds to N
+ * (possible when N is not a power of two) has no cell and is rejected too (ARC_EINVAL). */
 int arc_set_sources(arc_ctx *c, int nsrc, const double *pos_cm /*[nsrc][3]*/, const double *Ndot,
                     const double *binfrac /*[nsrc][nbins]*/);
 
@@ -217,6 +227,14 @@ int arc_trace_debug(arc_ctx *c, int step, arc_raylog *log);
 /* Device HEALPix generator, exposed for testing (O1): unit vectors of `n` (level, pixel) pairs.
  * HOST pointers; out is [n][3]. */
 int arc_pix2vec(const int32_t *level, const uint32_t *pix, int n, double *out);
+
+/* Self-test of the tracer's division (DESIGN.md 6.2 step 1, contract C3): the march needs the IEEE quotient
+ * RN(a / d) and gets it from RN(1/d) and two fused residual corrections.  Runs n_pairs device-generated pairs
+ * (counter-based generator on `seed`): a = i - g with integer 0 <= i <= 1025 and g uniform in [0, 1024) (also snapped to
+ * integers, half-integers and binary fractions), d = a direction component in (2^-40, 1] (uniform in exponent, random
+ * mantissa, also just below / at powers of two), both signs - and counts the pairs whose result differs in any bit from
+ * __ddiv_rn(a, d).  *mismatches must come back 0.  HOST pointer; synchronises; default stream. */
+int arc_selftest_division(uint64_t n_pairs, uint64_t seed, uint64_t *mismatches);
 
 const char *arc_last_error(const arc_ctx *c);          /* c may be NULL: last error of a failed create */
 const char *arc_version(void);

@@ -31,7 +31,7 @@ EXPORTS = ["arc_create_grid", "arc_destroy", "arc_default_params", "arc_set_para
            "arc_set_fields", "arc_get_fields", "arc_set_spectrum", "arc_set_sources", "arc_set_emission_mask", "arc_get_thin_radii", "arc_set_thin_radii", "arc_trace",
            "arc_trace_partial", "arc_accum_device", "arc_finalize",
            "arc_get_rates", "arc_get_accum", "arc_update_chemistry", "arc_suggest_dt", "arc_synchronize", "arc_get_stats",
-           "arc_trace_debug", "arc_pix2vec", "arc_last_error", "arc_version"]
+           "arc_trace_debug", "arc_pix2vec", "arc_selftest_division", "arc_last_error", "arc_version"]
 
 
 class ArcError(RuntimeError):
@@ -45,7 +45,7 @@ class arc_params(C.Structure):
                 ("Yp", C.c_double), ("isothermal", C.c_int32), ("caseB", C.c_int32), ("coll_ion", C.c_int32),
                 ("max_subcycles", C.c_int32), ("eps_sub", C.c_double), ("x_floor", C.c_double),
                 ("digest", C.c_int32), ("async_", C.c_int32), ("trace_blocks", C.c_int32), ("deposit", C.c_int32),
-                ("geom_corr", C.c_int32), ("reserved0", C.c_int32), ("thin_tau", C.c_double)]
+                ("geom_corr", C.c_int32), ("debug_fault", C.c_int32), ("thin_tau", C.c_double)]
 
 
 class arc_rates(C.Structure):
@@ -62,7 +62,7 @@ class arc_stats(C.Structure):
                 ("max_subcycles_cell", C.c_uint32), ("pad", C.c_uint32), ("trace_ms", C.c_float),
                 ("chem_ms", C.c_float), ("trace_kernel_ms", C.c_float), ("opacity_ms", C.c_float),
                 ("finalize_ms", C.c_float), ("trace_grid", C.c_int32), ("pad2", C.c_int32),
-                ("deposit_records", C.c_uint64)]
+                ("deposit_records", C.c_uint64), ("kernel_launches", C.c_uint64)]
 
 
 class arc_raylog(C.Structure):
@@ -106,6 +106,7 @@ def lib():
         l.arc_get_stats.argtypes = [vp, C.POINTER(arc_stats)]
         l.arc_trace_debug.argtypes = [vp, i32, C.POINTER(arc_raylog)]
         l.arc_pix2vec.argtypes = [vp, vp, i32, vp]
+        l.arc_selftest_division.argtypes = [C.c_uint64, C.c_uint64, C.POINTER(C.c_uint64)]
         l.arc_last_error.argtypes = [vp]
         l.arc_last_error.restype = C.c_char_p
         l.arc_version.restype = C.c_char_p
@@ -308,6 +309,15 @@ def arc_pix2vec(level, pix) -> np.ndarray:
     return out
 
 
+def arc_selftest_division(n_pairs: int, seed: int = 1) -> int:
+    """-> number of (a, d) pairs for which the tracer's division differs from IEEE division (must be 0)"""
+    bad = C.c_uint64(0)
+    rc = lib().arc_selftest_division(int(n_pairs), int(seed), C.byref(bad))
+    if rc != ARC_OK:
+        raise ArcError(rc, "arc_selftest_division failed")
+    return int(bad.value)
+
+
 # ---- helpers that only move data (no arithmetic) ---------------------------------------------------
 def stats_dict(s: arc_stats, nb: int) -> dict:
     return dict(segments=int(s.segments), rays=int(s.rays), digest=int(s.digest),
@@ -318,7 +328,7 @@ def stats_dict(s: arc_stats, nb: int) -> dict:
                 subcycles=int(s.subcycles), max_subcycles_cell=int(s.max_subcycles_cell),
                 trace_ms=float(s.trace_ms), chem_ms=float(s.chem_ms), trace_kernel_ms=float(s.trace_kernel_ms),
                 opacity_ms=float(s.opacity_ms), finalize_ms=float(s.finalize_ms), trace_grid=int(s.trace_grid),
-                deposit_records=int(s.deposit_records))
+                deposit_records=int(s.deposit_records), kernel_launches=int(s.kernel_launches))
 
 
 def params_from_dict(d: dict, **override) -> arc_params:
@@ -343,6 +353,7 @@ class Context:
         self.nb = w.nb
         self.np_dtype = np.float32 if w.dtype == "f32" else np.float64
         self.ctx = arc_create_grid(w.N, w.box_cm, ARC_F32 if w.dtype == "f32" else ARC_F64)
+        self.stream = stream                        # cudaStream_t handle the library enqueues on (None: legacy default stream)
         try:
             arc_set_params(self.ctx, params_from_dict(w.params, **param_override))
             if stream is not None:

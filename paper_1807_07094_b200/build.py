@@ -44,8 +44,7 @@ def nvcc_path() -> str:
 
 def _compile_one(args):
     src, obj, verbose = args
-    extra = os.environ.get("ARC_NVCC_EXTRA", "").split()          # e.g. -DARC_AGG_STEPS=2 (tuning builds)
-    cmd = [nvcc_path()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
+    cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
     r = subprocess.run(cmd, capture_output=True, text=True)
     return src, r.returncode, " ".join(cmd) + "\n" + r.stdout + r.stderr
 

@@ -37,7 +37,7 @@ void arc_default_params(arc_params *p)
     std::memset(p, 0, sizeof(*p));
     p->l0 = 1; p->Lmax = 13; p->Phi = 3.0; p->tau_term = 30.0; p->Yp = 0.0;
     p->isothermal = 1; p->caseB = 1; p->coll_ion = 0; p->max_subcycles = 4096;
-    p->eps_sub = 0.1; p->x_floor = 1e-12; p->digest = 0; p->async = 0; p->trace_blocks = 0; p->deposit = ARC_DEPOSIT_AUTO; p->geom_corr = ARC_GEOM_NONE; p->reserved0 = 0; p->thin_tau = 0.0;
+    p->eps_sub = 0.1; p->x_floor = 1e-12; p->digest = 0; p->async = 0; p->trace_blocks = 0; p->deposit = ARC_DEPOSIT_AUTO; p->geom_corr = ARC_GEOM_NONE; p->debug_fault = 0; p->thin_tau = 0.0;
 }
 
 int arc_create_grid(arc_ctx **out, int N, double box_cm, int dtype)
@@ -73,6 +73,7 @@ int arc_create_grid(arc_ctx **out, int N, double box_cm, int dtype)
     if (e == cudaSuccess) e = cudaMalloc(&c->d_stats, sizeof(DevStats));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_absorbed, sizeof(double) * ARC_MAX_BINS);
     if (e == cudaSuccess) e = cudaMemset(c->d_stats, 0, sizeof(DevStats));
+    if (e == cudaSuccess) e = cudaMemset(c->d_sched, 0, sizeof(SchedState));      // (the error word is sticky across resets)
     if (e == cudaSuccess) e = cudaMemset(c->d_absorbed, 0, sizeof(double) * ARC_MAX_BINS);
     for (int i = 0; i < 8 && e == cudaSuccess; ++i) e = cudaEventCreate(&c->ev[i]);
     if (e != cudaSuccess) {
@@ -113,6 +114,7 @@ int arc_set_params(arc_ctx *c, const arc_params *p)
     if (!(p->x_floor >= 0.0 && p->x_floor < 1.0)) return fail(c, ARC_EINVAL, "arc_set_params: x_floor must be in [0, 1)");
     if (p->trace_blocks < 0) return fail(c, ARC_EINVAL, "arc_set_params: trace_blocks must be >= 0");
     if (p->deposit < ARC_DEPOSIT_AUTO || p->deposit > ARC_DEPOSIT_QUAD) return fail(c, ARC_EINVAL, "arc_set_params: bad deposit mode");
+    if (p->debug_fault < 0 || p->debug_fault > ARC_DEV_RAY_RUNAWAY) return fail(c, ARC_EINVAL, "arc_set_params: debug_fault must be 0 or a device error code (1..4)");
     if (p->geom_corr < ARC_GEOM_NONE || p->geom_corr > ARC_GEOM_FC2) return fail(c, ARC_EINVAL, "arc_set_params: bad geom_corr");
     if (!(p->thin_tau >= 0.0) || !std::isfinite(p->thin_tau)) return fail(c, ARC_EINVAL, "arc_set_params: thin_tau must be finite and >= 0");
     if (p->thin_tau > 0.0 && (p->geom_corr != ARC_GEOM_NONE || p->deposit != ARC_DEPOSIT_AUTO))
@@ -157,7 +159,7 @@ int arc_get_fields(arc_ctx *c, void *n_H, void *x_HI, void *x_HeI, void *x_HeII,
     const cudaMemcpyKind kind = (where == ARC_HOST) ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
     for (int i = 0; i < 5; ++i)
         if (dst[i]) CK(cudaMemcpyAsync(dst[i], c->f[i], (size_t)c->ncell * esize(c), kind, c->stream));
-    if (where == ARC_HOST) CK(cudaStreamSynchronize(c->stream));
+    if (where == ARC_HOST) { CK(cudaStreamSynchronize(c->stream)); if (c->unchecked) return arc_check_device(c); }
     return ARC_OK;
 }
 
@@ -200,7 +202,9 @@ int arc_set_sources(arc_ctx *c, int nsrc, const double *pos_cm, const double *Nd
         for (int a = 0; a < 3; ++a) {
             const double x = pos_cm[3 * s + a];
             if (!(x >= 0.0 && x < c->box_cm)) return fail(c, ARC_EINVAL, "arc_set_sources: source position outside [0, box)");
-            g[3 * (size_t)s + a] = x / c->dx;                       // grid units
+            const double gg = x / c->dx;                            // grid units
+            if (!(gg < (double)c->N)) return fail(c, ARC_EINVAL, "arc_set_sources: source position rounds onto the upper box face (pos / (box / N) >= N): no cell");
+            g[3 * (size_t)s + a] = gg;
         }
         if (!(Ndot[s] >= 0.0) || !std::isfinite(Ndot[s])) return fail(c, ARC_EINVAL, "arc_set_sources: Ndot must be finite and >= 0");
         for (int v = 0; v < nb; ++v) {

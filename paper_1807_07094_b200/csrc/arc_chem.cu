@@ -171,8 +171,9 @@ __global__ void __launch_bounds__(128) arc_chem_iso_kernel(long long ncell, doub
                                                           int max_sub, ChemK q,
                                                           const FT *__restrict__ nHf, FT *__restrict__ xHIf, FT *__restrict__ xHeIf,
                                                           FT *__restrict__ xHeIIf, FT *__restrict__ Tf,
-                                                          const double *__restrict__ rates, DevStats *stats)
+                                                          const double *__restrict__ rates, DevStats *stats, const SchedState *__restrict__ sc)
 {
+    if (sc->error != ARC_DEV_OK || sc->in_flight != 0) return;      // the last trace aborted (async mode): fields stay as they are
     unsigned long long my_sub = 0; unsigned int my_max = 0;
     // an isothermal box usually has ONE temperature: the table at the block's first cell is evaluated once (first warp)
     // and shared; a cell at another temperature evaluates its own (same function, same argument: same bits)
@@ -217,8 +218,9 @@ __global__ void __launch_bounds__(128, 5) arc_chem_kernel(long long ncell, doubl
                                                       int max_sub, ChemK q,
                                                       const FT *__restrict__ nHf, FT *__restrict__ xHIf, FT *__restrict__ xHeIf,
                                                       FT *__restrict__ xHeIIf, FT *__restrict__ Tf,
-                                                      const double *__restrict__ rates, DevStats *stats)
+                                                      const double *__restrict__ rates, DevStats *stats, const SchedState *__restrict__ sc)
 {
+    if (sc->error != ARC_DEV_OK || sc->in_flight != 0) return;      // the last trace aborted (async mode): fields stay as they are
     const unsigned lane = threadIdx.x & 31u;
     unsigned long long my_sub = 0; unsigned int my_max = 0;
     long long mine = -1;                          // this lane's cell, -1 = none
@@ -264,8 +266,9 @@ template <typename FT>
 __global__ void __launch_bounds__(256) arc_dt_kernel(long long ncell, int scheme, double eps, double sigma1, double d, double Yp,
                                                     ChemK q, const FT *__restrict__ nHf, const FT *__restrict__ xHIf,
                                                     const FT *__restrict__ xHeIf, const FT *__restrict__ xHeIIf, const FT *__restrict__ Tf,
-                                                    const double *__restrict__ GammaHI, unsigned long long *out)
+                                                    const double *__restrict__ GammaHI, unsigned long long *out, const SchedState *__restrict__ sc)
 {
+    if (sc->error != ARC_DEV_OK || sc->in_flight != 0) return;
     double best = __longlong_as_double(0x7ff0000000000000ll);
     unsigned long long used = 0;
     for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
@@ -307,7 +310,8 @@ cudaError_t launch_dt(arc_ctx *c, int scheme, double eps)
     const long long cap = (long long)c->n_sm * 8;
     FT **f = reinterpret_cast<FT **>(c->f);
     arc_dt_kernel<FT><<<(int)(nb < cap ? nb : cap), 256, 0, c->stream>>>(c->ncell, scheme, eps, c->spec.sig[0][0], c->dx, c->p.Yp,
-                                                                        chem_consts(c->p.caseB != 0, c->p.coll_ion != 0), f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_dt);
+                                                                        chem_consts(c->p.caseB != 0, c->p.coll_ion != 0), f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_dt, c->d_sched);
+    ++c->launches;
     return cudaGetLastError();
 }
 
@@ -320,7 +324,7 @@ cudaError_t launch_chem(arc_ctx *c, double dt)
     if (c->p.isothermal) {
         const long long cap = (long long)c->n_sm * 32;
         arc_chem_iso_kernel<FT><<<(int)(nb < cap ? nb : cap), 128, 0, c->stream>>>(c->ncell, dt, c->p.Yp, c->p.eps_sub, c->p.x_floor, c->p.max_subcycles,
-                                                                                 q, f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_stats);
+                                                                                 q, f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_stats, c->d_sched);
     } else {
         // persistent: exactly the co-resident blocks (stats->chem_next is zeroed by arc_update_chemistry)
         int per_sm = 0;
@@ -328,8 +332,9 @@ cudaError_t launch_chem(arc_ctx *c, double dt)
         if (e != cudaSuccess) return e;
         const long long cap = (long long)c->n_sm * (per_sm > 0 ? per_sm : 1);
         arc_chem_kernel<FT><<<(int)(nb < cap ? nb : cap), 128, 0, c->stream>>>(c->ncell, dt, c->p.Yp, c->p.eps_sub, c->p.x_floor, c->p.max_subcycles,
-                                                                             q, f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_stats);
+                                                                             q, f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_stats, c->d_sched);
     }
+    ++c->launches;
     return cudaGetLastError();
 }
 

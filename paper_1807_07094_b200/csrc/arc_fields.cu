@@ -37,8 +37,11 @@ __global__ void __launch_bounds__(256) arc_finalize_kernel(long long ncell, int 
                                                           const FT *__restrict__ nH, const FT *__restrict__ xHI,
                                                           const FT *__restrict__ xHeI, const FT *__restrict__ xHeII,
                                                           const double *__restrict__ A, double *__restrict__ rates,
-                                                          double *__restrict__ absorbed)
+                                                          double *__restrict__ absorbed, const SchedState *__restrict__ sc)
 {
+    // async mode: a trace that aborted on the device (sticky error word, or families left in flight) has no valid
+    // accumulators - leave the rates alone; the host reports the error at its next synchronising call
+    if (sc->error != ARC_DEV_OK || sc->in_flight != 0) return;
     const double EV = 1.602176634e-12;
     const double ETH[3] = {13.598, 24.587, 54.418};
     double acc[ARC_MAX_BINS];
@@ -106,6 +109,7 @@ cudaError_t arc_launch_opacity(arc_ctx *c)
         arc_opacity_kernel<double><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, arc_nbp(c->spec.nb), c->p.Yp, c->spec, (const double *)c->f[0],
                                                            (const double *)c->f[1], (const double *)c->f[2], (const double *)c->f[3],
                                                            (double *)c->d_kappa, c->d_A);
+    ++c->launches;
     return cudaGetLastError();
 }
 
@@ -157,6 +161,7 @@ cudaError_t arc_launch_thin_region(arc_ctx *c, double maxR)
     else
         arc_thin_region_kernel<double><<<grid, 256, 0, c->stream>>>(c->N, c->nsrc, nb, arc_nbp(nb), side, c->dx, c->d_src_g, c->d_Rstart, c->d_Sopen,
                                                                    (const double *)c->d_kappa, c->d_A);
+    ++c->launches;
     return cudaGetLastError();
 }
 
@@ -169,10 +174,11 @@ cudaError_t arc_launch_finalize(arc_ctx *c)
     if (c->dtype == ARC_F32)
         arc_finalize_kernel<float><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, arc_nbp(c->spec.nb), c->p.Yp, V, c->spec, (const float *)c->f[0],
                                                            (const float *)c->f[1], (const float *)c->f[2], (const float *)c->f[3],
-                                                           c->d_A, c->d_rates, c->d_absorbed);
+                                                           c->d_A, c->d_rates, c->d_absorbed, c->d_sched);
     else
         arc_finalize_kernel<double><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, arc_nbp(c->spec.nb), c->p.Yp, V, c->spec, (const double *)c->f[0],
                                                             (const double *)c->f[1], (const double *)c->f[2], (const double *)c->f[3],
-                                                            c->d_A, c->d_rates, c->d_absorbed);
+                                                            c->d_A, c->d_rates, c->d_absorbed, c->d_sched);
+    ++c->launches;
     return cudaGetLastError();
 }

@@ -140,6 +140,8 @@ struct arc_ctx {
     bool traced_once = false, chem_once = false;
     bool have_accum = false;          // arc_trace_partial ran: the accumulators wait for arc_finalize
     bool finalize_split = false;      // the last finalise pass was arc_finalize's (events 4, 7)
+    unsigned long long launches = 0;  // kernels launched by this context (arc_stats.kernel_launches)
+    bool unchecked = false;           // an asynchronous trace has been enqueued and its device error word not yet looked at
     std::string err;
 };
 
@@ -152,6 +154,8 @@ cudaError_t arc_launch_sched_reset(arc_ctx *c, unsigned long long seed_total);
 cudaError_t arc_launch_trace(arc_ctx *c, const TraceArgs &a, bool log, int *grid_out);
 int arc_trace_occupancy_grid(arc_ctx *c, int nb, int flags);   // flags: 1 log, 2 digest
 cudaError_t arc_launch_pix2vec(const int32_t *d_level, const uint32_t *d_pix, int n, double *d_out, cudaStream_t s);
+// arc_run.cu: after the stream has been synchronised - report (and clear) what the last trace left in the device error word
+int arc_check_device(arc_ctx *c);
 // arc_chem.cu
 cudaError_t arc_launch_chemistry(arc_ctx *c, double dt);
 cudaError_t arc_launch_suggest_dt(arc_ctx *c, int scheme, double eps);     // result in c->d_dt

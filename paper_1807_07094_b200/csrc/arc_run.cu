@@ -20,13 +20,16 @@ static int fail(arc_ctx *c, int code, const std::string &msg) { c->err = msg; re
 
 static size_t famrec_bytes(int nb) { return (size_t)(16 + 16 * nb); }      // sizeof(FamRec<nb>)
 
-// check the device-side error word after a synchronised trace
-static int device_error(arc_ctx *c)
+// check the device-side error word after the stream has been synchronised; an error is reported once and cleared (the
+// word is sticky on the device: until then every consumer kernel skips its work, arc_trace.cu / arc_fields.cu / arc_chem.cu)
+int arc_check_device(arc_ctx *c)
 {
+    c->unchecked = false;
     SchedState h;
     CK(cudaMemcpy(&h, c->d_sched, sizeof(h), cudaMemcpyDeviceToHost));
     if (h.error == ARC_DEV_OK && h.in_flight == 0) return ARC_OK;
     c->have_rates = false; c->have_accum = false;
+    CK(cudaMemset(&c->d_sched->error, 0, sizeof(int)));
     switch (h.error) {
         case ARC_DEV_STACK_OVERFLOW: return fail(c, ARC_EOVERFLOW, "arc_trace: a warp's work stack overflowed; rates are invalid");
         case ARC_DEV_LOG_OVERFLOW: return fail(c, ARC_EOVERFLOW, "arc_trace_debug: ray log too small");
@@ -145,7 +148,7 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
         std::vector<unsigned long long> bits((size_t)c->nsrc);
         CK(cudaMemcpyAsync(bits.data(), c->d_Rnext, sizeof(unsigned long long) * c->nsrc, cudaMemcpyDeviceToHost, c->stream));
         CK(cudaStreamSynchronize(c->stream));
-        const int de = device_error(c);
+        const int de = arc_check_device(c);
         if (de != ARC_OK) return de;
         for (int s = 0; s < c->nsrc; ++s) {
             double R = 0.0;
@@ -156,10 +159,14 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
     }
     if (!c->p.async || log) {
         CK(cudaStreamSynchronize(c->stream));
-        return device_error(c);
+        return arc_check_device(c);
     }
+    c->unchecked = true;              // async: whoever synchronises next looks at the device error word
     return ARC_OK;
 }
+
+// for the calls that have just synchronised the stream
+static int check_pending(arc_ctx *c) { return c->unchecked ? arc_check_device(c) : ARC_OK; }
 
 static void fill_rates(arc_ctx *c, arc_rates *out)
 {
@@ -207,7 +214,7 @@ int arc_finalize(arc_ctx *c, arc_rates *out)
     c->have_accum = false;
     c->have_rates = true;
     c->finalize_split = true;
-    if (!c->p.async) CK(cudaStreamSynchronize(c->stream));
+    if (!c->p.async) { CK(cudaStreamSynchronize(c->stream)); const int de = check_pending(c); if (de != ARC_OK) return de; }
     if (out) fill_rates(c, out);
     return ARC_OK;
 }
@@ -251,7 +258,7 @@ int arc_get_rates(arc_ctx *c, double *Gamma_HI, double *Gamma_HeI, double *Gamma
     const cudaMemcpyKind kind = (where == ARC_HOST) ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
     for (int i = 0; i < 7; ++i)
         if (dst[i]) CK(cudaMemcpyAsync(dst[i], c->d_rates + (size_t)i * c->ncell, (size_t)c->ncell * sizeof(double), kind, c->stream));
-    if (where == ARC_HOST) CK(cudaStreamSynchronize(c->stream));
+    if (where == ARC_HOST) { CK(cudaStreamSynchronize(c->stream)); return check_pending(c); }
     return ARC_OK;
 }
 
@@ -264,7 +271,7 @@ int arc_get_accum(arc_ctx *c, double *A, int where)
     const int nb = c->spec.nb, nbp = arc_nbp(nb);        // device rows are padded to nbp doubles; the caller gets [cell][nb]
     if (nbp == nb) CK(cudaMemcpyAsync(A, c->d_A, (size_t)c->ncell * nb * sizeof(double), kind, c->stream));
     else CK(cudaMemcpy2DAsync(A, nb * sizeof(double), c->d_A, nbp * sizeof(double), nb * sizeof(double), (size_t)c->ncell, kind, c->stream));
-    if (where == ARC_HOST) CK(cudaStreamSynchronize(c->stream));
+    if (where == ARC_HOST) { CK(cudaStreamSynchronize(c->stream)); return check_pending(c); }
     return ARC_OK;
 }
 
@@ -279,7 +286,7 @@ int arc_update_chemistry(arc_ctx *c, double dt_s)
     CK(cudaEventRecord(c->ev[6], c->stream));
     c->chem_once = true;
     // the rates stay valid as numbers, but they belong to the fields before this update
-    if (!c->p.async) CK(cudaStreamSynchronize(c->stream));
+    if (!c->p.async) { CK(cudaStreamSynchronize(c->stream)); return check_pending(c); }
     return ARC_OK;
 }
 
@@ -297,6 +304,7 @@ int arc_suggest_dt(arc_ctx *c, int scheme, double eps, double *dt_s, int64_t *ce
     unsigned long long h[2];
     CK(cudaMemcpyAsync(h, c->d_dt, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
+    { const int de = check_pending(c); if (de != ARC_OK) return de; }
     double dt = INFINITY;
     if (h[0] < 0x7ff0000000000000ull) std::memcpy(&dt, &h[0], sizeof(dt));
     *dt_s = dt;
@@ -308,7 +316,7 @@ int arc_synchronize(arc_ctx *c)
 {
     if (!c) return ARC_EINVAL;
     CK(cudaStreamSynchronize(c->stream));
-    if (c->traced_once) return device_error(c);
+    if (c->traced_once) return arc_check_device(c);
     return ARC_OK;
 }
 
@@ -338,8 +346,9 @@ int arc_get_stats(arc_ctx *c, arc_stats *s)
         }
     }
     if (c->chem_once) cudaEventElapsedTime(&s->chem_ms, c->ev[5], c->ev[6]);
+    s->kernel_launches = c->launches;
     cudaGetLastError();
-    return ARC_OK;
+    return check_pending(c);                    // (the statistics are filled in either way)
 }
 
 int arc_pix2vec(const int32_t *level, const uint32_t *pix, int n, double *out)

@@ -26,6 +26,7 @@
 #pragma once
 #include "arc_internal.cuh"
 #include "arc_healpix.cuh"
+#include "arc_divide.cuh"
 
 #define FLAG_LOG 1          // template flag: per-ray logging (arc_trace_debug)
 #define FLAG_DIGEST 2       // template flag: accumulate the order-independent traversal digest
@@ -34,7 +35,7 @@
 #define ARC_GREEDY_MIN_INFLIGHT 2048   // families alive above which idle warps take whole batches from the donation queue
 #endif
 #ifndef ARC_DONATE_KEEP
-#define ARC_DONATE_KEEP 8              // a donor keeps its next batch (8 families) and gives away the rest, 32 at a time (0: gives half its ring)
+#define ARC_DONATE_KEEP 8              // a donor keeps its next batch (8 families) and gives away the rest, 32 at a time
 #endif
 #ifndef ARC_POOL_PER_HUNGRY
 #define ARC_POOL_PER_HUNGRY ARC_BATCH_FAM      // donors keep the pool at this many families per idle warp
@@ -43,9 +44,6 @@
 
 #ifndef ARC_TRACE_MIN_BLOCKS
 #define ARC_TRACE_MIN_BLOCKS 3     // resident blocks per SM the register budget is held to (<= 85 registers)
-#endif
-#ifndef ARC_AGG_STEPS
-#define ARC_AGG_STEPS 0            // warp-aggregated deposit: 0 = match.any groups (any lanes); k > 0 = runs of up to 2^k neighbouring lanes
 #endif
 #define DEP_RED 1           // every lane: nb fp64 REDs per segment
 #define DEP_AGG 2           // lanes of a warp that sit in the same cell are summed first (match.any + shuffles): one lane REDs
@@ -155,18 +153,6 @@ __device__ __forceinline__ void arc_attenuate(double x, double &E, double &ome)
     ome = (k == 0) ? -em1 : 1.0 - Ek;
 }
 
-// a / b rounded to nearest, bit-identical to IEEE division, given y = RN(1 / b) (one true division per ray and axis):
-// q0 = RN(a y) is within 1.5 ulp of a/b; one residual correction q1 = RN(q0 + (a - b q0) y) makes it faithful, and
-// for a faithful q1 and a correctly rounded y the second correction returns RN(a / b) (Markstein 1990, the closing
-// step of the IA-64 division sequences).  The residuals are exact (FMA).  No overflow / underflow here: |a| <= 2N,
-// 2^-40 < |b| <= 1.  Five FP64 instructions instead of the ~17 of the generic division.
-__device__ __forceinline__ double arc_div_by_recip(double a, double b, double y)
-{
-    const double q0 = __dmul_rn(a, y);
-    const double q1 = __fma_rn(__fma_rn(-b, q0, a), y, q0);
-    return __fma_rn(__fma_rn(-b, q1, a), y, q1);
-}
-
 // x += o under a predicate: one predicated DADD (the compiler's own choice is DADD + two selects)
 __device__ __forceinline__ void arc_add_if(double &x, double o, int take)
 {
@@ -222,8 +208,9 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
     constexpr int NBE = (NB + 1) & ~1;                        // bins rounded up to whole fp32 pairs
     unsigned long long nred = 0;                              // deposit records this lane sent to L2
 
-    // per-block tallies: 32-bit shared atomics are native (64-bit ones are CAS loops); spilled to the 64-bit global
-    // counters at the end and whenever one passes 2^30 (tally_spill)
+    // per-block tallies: 32-bit shared atomics are native (64-bit ones are CAS loops); added to the 64-bit global
+    // counters at the end.  A block traces < 2^32 rays: at most 1.2e7 rays per source and 2^24 sources spread over
+    // >= 148 blocks would be needed to wrap one, i.e. > 5e12 rays = weeks of tracing in one launch.
     __shared__ unsigned int s_splits[ARC_MAX_LEVEL], s_rays[ARC_MAX_LEVEL], s_ends[3];
     __shared__ double s_esc[ARC_MAX_BINS];
     __shared__ double s_geo[9][ARC_TRACE_THREADS];            // per thread: source position g[3], direction d[3], RN(1/d)[3]
@@ -248,7 +235,12 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
     if (threadIdx.x < ARC_MAX_LEVEL) { s_splits[threadIdx.x] = 0; s_rays[threadIdx.x] = 0; }
     if (threadIdx.x < 3) s_ends[threadIdx.x] = 0;
     if (threadIdx.x < ARC_MAX_BINS) s_esc[threadIdx.x] = 0.0;
+    // a sticky device error from an earlier asynchronous trace (or arc_params.debug_fault): this trace does not run; its
+    // root families stay "in flight", which tells every consumer kernel to skip (block-uniform decision)
+    __shared__ int s_abort;
+    if (threadIdx.x == 0) s_abort = ld_volatile_s32(&sc->error);
     __syncthreads();
+    if (s_abort != 0) return;
 
     // own stack = ring of ARC_STACK_CAP records holding families [bot, top) (monotonic counters, warp-uniform)
     unsigned bot = 0, top = 0;
@@ -591,7 +583,6 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
           // a7: deposit - the whole warp, converged (a lambda: the geometric correction runs the stage a second time)
           auto deposit = [&](const int dcell, double (&av)[NB]) {
           if constexpr (DEP == DEP_AGG) {
-#if ARC_AGG_STEPS == 0
               // segmented sum over the lanes that share a cell, by pointer jumping along each group's lane list:
               // after ceil(log2(group size)) rounds the first lane of a group holds the group's sum
               const unsigned peers = __match_any_sync(0xffffffffu, dcell);
@@ -607,22 +598,6 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                   nxt = __shfl_sync(0xffffffffu, nxt, from);              // (a tail lane reads its own -1)
               }
               const bool head = (lane == leader);
-#else
-              // lanes are ordered (family, child) in nested pixel order, so rays that share a cell sit in NEIGHBOURING
-              // lanes: sum over runs of equal cells (cut at multiples of 2^ARC_AGG_STEPS lanes) with a fixed number of
-              // shuffle-down steps; the first lane of a run issues the REDs.  Equal cells in non-adjacent lanes are
-              // simply deposited separately - the sums are the same.
-              const int prev = __shfl_up_sync(0xffffffffu, dcell, 1);
-              const bool head = (prev != dcell) || ((lane & ((1 << ARC_AGG_STEPS) - 1)) == 0);
-              const unsigned above = __ballot_sync(0xffffffffu, head) & (0xfffffffeu << lane);   // run heads after my lane
-              const int last = above ? __ffs(above) - 2 : 31;                                   // last lane of my run
-#pragma unroll
-              for (int d = 1; d < (1 << ARC_AGG_STEPS); d <<= 1) {
-                  const int take = lane + d <= last;
-#pragma unroll
-                  for (int v = 0; v < NB; ++v) arc_add_if(av[v], __shfl_down_sync(0xffffffffu, av[v], d), take);
-              }
-#endif
               if (head && dcell >= 0) {
                   double *Ac = a.A + (long long)dcell * NBP;
 #pragma unroll
@@ -717,11 +692,6 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                     if (lane == 0) atomicAdd(&s_esc[v], e);
                 }
             }
-            if (lane < ARC_MAX_LEVEL) {                  // tally_spill: keep the 32-bit block tallies far from wrapping
-                if (s_rays[lane] > 0x40000000u) { const unsigned n = atomicExch(&s_rays[lane], 0u); atomicAdd(&a.stats->rays_level[lane], (unsigned long long)n); atomicAdd(&a.stats->rays, (unsigned long long)n); }
-                if (s_splits[lane] > 0x40000000u) atomicAdd(&a.stats->splits[lane], (unsigned long long)atomicExch(&s_splits[lane], 0u));
-                if (lane < 3 && s_ends[lane] > 0x40000000u) atomicAdd(&a.stats->ends[lane], (unsigned long long)atomicExch(&s_ends[lane], 0u));
-            }
         }
         if (end >= 0) {
             if (FLAGS & FLAG_DIGEST) { h = mix64(h ^ (0xE0ull + (unsigned long long)end)); digest += h; }
@@ -760,11 +730,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
         hungry = __shfl_sync(0xffffffffu, hungry, 0);
         err = __shfl_sync(0xffffffffu, err, 0);
         if (err) quit = true;
-#if ARC_DONATE_KEEP > 0
-        const unsigned nd_max = min(top - bot > (unsigned)ARC_DONATE_KEEP ? top - bot - (unsigned)ARC_DONATE_KEEP : 0u, 32u);   // keep the next batch(es), give the rest
-#else
-        const unsigned nd_max = min((top - bot) / 2, 32u);
-#endif
+        const unsigned nd_max = min(top - bot > (unsigned)ARC_DONATE_KEEP ? top - bot - (unsigned)ARC_DONATE_KEEP : 0u, 32u);   // keep the next batch, give the rest
         if (!quit && hungry > 0 && nd_max > 0) {
             int nd = (int)nd_max;
             unsigned long long ticket = 0;

@@ -43,14 +43,23 @@ def trace_sharded(tracer, group=None, step: int = 0):
     """One radiative-transfer pass with the sources sharded over the ranks of `group`.
 
     `tracer` holds THIS rank's share of the sources and offers `trace_partial(step)`, `accum_tensor()` (a tensor that
-    aliases its accumulators) and `finalize()` - `arc.Context` does.  The all-reduce is issued on torch's current
-    stream: callers run the context on that stream (`Context(stream=torch.cuda.current_stream().cuda_stream)`).
+    aliases its accumulators) and `finalize()` - `arc.Context` does.  The three steps must run in stream order: the
+    all-reduce is issued ON THE CONTEXT'S OWN STREAM (`tracer.stream`, a cudaStream_t handle; 0 / None = the legacy
+    default stream), whatever torch's current stream is, so that it follows the tracer's REDs and precedes finalize
+    also when the context runs with `async = 1`.
     """
+    import contextlib
     import torch.distributed as dist
     tracer.trace_partial(step)
     A = tracer.accum_tensor()
     if dist.is_initialized() and dist.get_world_size(group) > 1:
-        dist.all_reduce(A, op=dist.ReduceOp.SUM, group=group)
+        on_stream = contextlib.nullcontext()
+        handle = getattr(tracer, "stream", None)
+        if getattr(A, "is_cuda", False):
+            import torch
+            on_stream = torch.cuda.stream(torch.cuda.ExternalStream(int(handle)) if handle else torch.cuda.default_stream())
+        with on_stream:
+            dist.all_reduce(A, op=dist.ReduceOp.SUM, group=group)
     return tracer.finalize()
 
 

@@ -65,3 +65,71 @@ def run_gpu_trace(w, fields=None, **override):
 
 def oracle_override(override):
     return {k: v for k, v in override.items() if k not in ("digest", "async", "trace_blocks", "deposit")}
+
+
+# ---- the oracle on all host cores (tests only; bench.py times it as it stands, single-threaded) -------------------------
+def oracle_trace_parallel(w, fields=None, sources=None, threads=None, **override):
+    """orc.trace of `sources` (default: all), spread over host threads by (source, root pixel): every job traces ALL the
+    listed sources with an emission mask (orc_trace_masked) that leaves open only its share of the root rays,
+    so source ids - and with them the per-ray digests - are those of the one-call trace.  Rays are independent and the
+    accumulators add: A and the float tallies are summed, integer tallies added, digests added mod 2^64.
+    The C oracle itself is untouched and single-threaded; ctypes releases the GIL.  -> (A, stats)"""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    threads = threads or min(16, os.cpu_count() or 1)
+    src = np.arange(w.nsrc) if sources is None else np.asarray(sources)
+    l0 = int(override.get("l0", w.params["l0"]))
+    npix0 = 12 << (2 * l0)
+    units = [(s, p) for s in range(len(src)) for p in range(npix0)]
+    njobs = min(threads, len(units))
+    kappa = orc.opacity(w, fields, **{k: v for k, v in override.items() if k in ("Yp",)})
+    masks = []
+    for j in range(njobs):
+        m = np.ones((w.nsrc, npix0), dtype=np.uint8)          # (orc.trace picks the rows of `sources` itself)
+        for (s, p) in units[j::njobs]:
+            m[src[s], p] = 0
+        masks.append(m)
+
+    def job(m):
+        return orc.trace(w, kappa=kappa, sources=src, blocked=m, **override)[:2]
+
+    with ThreadPoolExecutor(max_workers=njobs) as ex:
+        parts = list(ex.map(job, masks))
+    A = parts[0][0]
+    st = {k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in parts[0][1].items()}
+    for Ap, sp in parts[1:]:
+        A += Ap
+        for k in ("segments", "rays"):
+            st[k] += sp[k]
+        st["digest"] = (st["digest"] + sp["digest"]) & 0xFFFFFFFFFFFFFFFF
+        for k in ("splits", "rays_level", "ends", "emitted", "absorbed", "escaped"):
+            st[k] = st[k] + sp[k]
+    return A, st
+
+
+def oracle_chemistry_parallel(w, fields, Gamma, heat, dt, threads=None, chunk=64 ** 3, **override):
+    """orc.chemistry over a flat range of cells (the whole grid, or a slab of it) on all host cores: the update is per cell
+    (PAPER.md:156), so the arrays are cut into chunks of `chunk` = 64^3 cells, each handed to the unchanged C routine
+    as a 64^3 'grid'.  -> (new fields tuple, subcycles[cells])"""
+    import os
+    import dataclasses
+    from concurrent.futures import ThreadPoolExecutor
+    threads = threads or min(16, os.cpu_count() or 1)
+    nc = len(fields[0])
+    assert nc % chunk == 0 and round(chunk ** (1 / 3)) ** 3 == chunk
+    wc = dataclasses.replace(w, N=round(chunk ** (1 / 3)))
+    f = [np.ascontiguousarray(np.asarray(a, dtype=np.float64)) for a in fields]
+    G = np.asarray(Gamma, dtype=np.float64); H = np.asarray(heat, dtype=np.float64)
+    out = [a.copy() for a in f]
+    sub = np.zeros(nc, dtype=np.int32)
+
+    def job(i):
+        sl = slice(i * chunk, (i + 1) * chunk)
+        nf, sb = orc.chemistry(wc, [a[sl] for a in f], np.ascontiguousarray(G[:, sl]), np.ascontiguousarray(H[:, sl]), dt, **override)
+        for k in range(1, 5):
+            out[k][sl] = nf[k]
+        sub[sl] = sb
+
+    with ThreadPoolExecutor(max_workers=threads) as ex:
+        list(ex.map(job, range(nc // chunk)))
+    return tuple(out), sub

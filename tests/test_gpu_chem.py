@@ -33,22 +33,18 @@ def test_one_step_random_cells(dtype, iso, Yp, nb):
     compare_trace_stats(st, ref["stats"], nb, RTOL[dtype])
     assert_close(G, ref["Gamma"], RTOL[dtype], "Gamma")
     assert_close(H, ref["heat"], RTOL[dtype], "heat")
-    # (a) the update itself, given the SAME rates (the CUDA path's) on both sides: every cell within the bar
-    same_rates, _ = orc.chemistry(w, w.fields(), G, H, w.dt_s)
+    # The update itself, given the SAME rates (the CUDA path's) on both sides: every cell within the bar, no allowance.
+    # Together with the rates above (within the bar, every cell) this IS whole-step parity: what is left between the
+    # CUDA path's step and the oracle's own step is orc(G_gpu) - orc(G_oracle), the oracle's response to a
+    # within-tolerance change of its own inputs - large in a few cells, because the sub-cycle limiter as printed
+    # (reading G15) makes the update ill-conditioned where heat - cool changes sign
+    # (tests/test_oracle_chem.py::test_update_is_ill_conditioned_where_the_limiter_switches shows it on the CPU alone).
+    same_rates, sub = orc.chemistry(w, w.fields(), G, H, w.dt_s)
     _fields_close(got, same_rates, dtype, what="same rates: ")
-    # (b) whole step against the oracle's own step.  The sub-cycle limiter as printed (reading G15) makes
-    # the update a discontinuous function of the rates: where heat - cool changes sign, or where the time left is
-    # about one limiter step, a 1e-7 change in a rate changes the NUMBER of sub-steps and with it the first-order
-    # truncation error.  So: every cell within 10x the bar, and all but 0.5 % of the cells within the bar.
-    for n, g, o in zip(("x_HI", "x_HeI", "x_HeII", "T"), got[1:], ref["fields"][1:]):
-        assert_close(g, o, 10 * RTOL[dtype], f"whole step {n}")
-        g = np.asarray(g, np.float64); o = np.asarray(o, np.float64)
-        off = np.abs(g - o) > RTOL[dtype] * np.maximum(np.abs(g), np.abs(o)) + 1e-12 * np.abs(o).max()
-        assert off.mean() <= 0.005, f"whole step {n}: {int(off.sum())} of {off.size} cells outside the bar"
     # sub-cycle counts: decided by floating-point limiters, so equal up to a handful of cells
-    tot = int(ref["subcycles"].sum())
-    assert abs(st2["subcycles"] - tot) <= max(4, tot // 1000), (st2["subcycles"], tot)
-    assert st2["max_subcycles_cell"] >= 1
+    tot = int(sub.sum())
+    assert abs(st2["subcycles"] - tot) <= max(4, tot // 10000), (st2["subcycles"], tot)
+    assert st2["max_subcycles_cell"] == int(sub.max())
 
 
 def test_chemistry_with_injected_rates_matches_cell_by_cell():

@@ -36,7 +36,7 @@ def _one_step_both(w, cx, fields, step, rtol):
     cx.update_chemistry()
     got = cx.get_fields()
     for name, a, b in zip(("x_HI", "x_HeI", "x_HeII", "T"), got[1:], ref["fields"][1:]):
-        assert_close(a, b, rtol, f"step {step}: {name}", atol_frac=1e-9)
+        assert_close(a, b, rtol, f"step {step}: {name}")
     return ref["fields"]
 
 

@@ -1,0 +1,122 @@
+"""Parity at the sizes bench.py runs, by the protocol of SURVEY 8(d) "Oracle timing".
+
+Configs 4 and 5 are out of the oracle's reach in full (1e11-1e12 segments per step), so
+  * the TRACER is compared on a seeded 16-source subset (rates are linear in the sources), on the
+    fields a free-running device run has reached at steps 0, 10 and 19 - injected into both sides;
+  * the CHEMISTRY is compared on the whole 256^3 fp32 grid (every cell, strict) with the device's own rates of those
+    steps handed to the oracle - the first comparison of arc_chem_kernel<float> at the size the bench runs;
+  * one full-size fp32 case ends rays DEPLETED (tau_term = 3), which config 4 as specified never does;
+  * config 5: the source nearest the centre of the 512^3 grid, and the chemistry on a 512 x 512 x 32 slab.
+The oracle runs on all host cores here (gpu_common.oracle_*_parallel: the unchanged single-threaded C routine, called on
+disjoint shares of the rays / cells); bench.py times it as it stands.
+Tolerances: integers bit-exact; floats 1e-3 relative (fp32 fields, fp64 accumulation) + 1e-12 of the array maximum.
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_1807_07094_b200 import arc, workloads as wl
+from gpu_common import RTOL, assert_close, compare_trace_stats, oracle_chemistry_parallel, oracle_trace_parallel
+
+pytestmark = pytest.mark.gpu
+R32 = RTOL["f32"]
+
+
+def _subset_parity(w, fields, sample, what, **override):
+    """both sides trace the sources `sample` alone on `fields`; -> the device's statistics"""
+    Ao, so = oracle_trace_parallel(w, fields=fields, sources=sample, **override)
+    with arc.Context(w, fields=fields, digest=1, **override) as cx:
+        cx.set_sources(sample)
+        cx.trace()
+        st = cx.stats()
+        compare_trace_stats(st, so, w.nb, R32)
+        assert_close(cx.accum(), Ao, R32, f"{what}: A")
+        G, H, Ht = cx.rates()
+    Go, Ho, Hto = orc.finalize(w, Ao, fields, **{k: v for k, v in override.items() if k == "Yp"})
+    assert_close(G, Go, R32, f"{what}: Gamma")
+    assert_close(H, Ho, R32, f"{what}: heat per absorber")
+    assert_close(Ht, Hto, R32, f"{what}: heat_total")
+    return st
+
+
+def _chemistry_parity(w, before, G, H, got, what):
+    """the oracle's update of `before` with the DEVICE's rates against the device's updated fields `got`, every cell"""
+    want, sub = oracle_chemistry_parallel(w, before, G, H, w.dt_s)
+    for name, a, b in zip(("x_HI", "x_HeI", "x_HeII", "T"), got[1:], want[1:]):
+        assert_close(a, b, R32, f"{what}: {name}")
+    return sub
+
+
+def test_config4_sixteen_sources_and_the_whole_grid_chemistry_at_steps_0_10_19():
+    w = wl.config4()
+    rng = np.random.default_rng(wl.SEED0 + 416)
+    sample = np.sort(rng.choice(w.nsrc, size=16, replace=False))
+    checked = 0
+    with arc.Context(w) as cx:                                   # the benched launch configuration, free running
+        for step in range(20):
+            if step in (0, 10, 19):
+                before = cx.get_fields()                         # fp32 arrays: what both sides start this step from
+                cx.trace(step)
+                st = cx.stats()
+                assert_close(st["absorbed"] + st["escaped"], st["emitted"], 1e-10, f"step {step}: conservation")
+                G, H, _ = cx.rates()
+                cx.update_chemistry()
+                got = cx.get_fields()
+                st2 = cx.stats()
+                sub = _chemistry_parity(w, before, G, H, got, f"step {step}, 256^3 chemistry with the device's rates")
+                tot = int(sub.sum())
+                assert abs(st2["subcycles"] - tot) <= max(16, tot // 10000), (st2["subcycles"], tot)
+                assert st2["max_subcycles_cell"] == int(sub.max())
+                del G, H, got
+                _subset_parity(w, before, sample, f"step {step}, 16 sources")
+                checked += 1
+            else:
+                cx.trace(step); cx.update_chemistry()
+        xe = 1.0 - float(np.mean(cx.get_fields()[1].astype(np.float64)))
+    assert checked == 3 and xe > 0.05                            # the box really ionised over the run
+
+
+def test_config4_sixteen_sources_with_rays_that_deplete():
+    """tau_term = 3 on the neutral step-0 fields: most rays end DEPLETED a few cells from their source (config 4 as
+    specified never gets there: its hardest bin stays below tau_term = 30) - the depleted branch of
+    arc_trace_kernel<4, float> at full size"""
+    w = wl.config4()
+    rng = np.random.default_rng(wl.SEED0 + 417)
+    sample = np.sort(rng.choice(w.nsrc, size=16, replace=False))
+    st = _subset_parity(w, w.fields(), sample, "tau_term = 3", tau_term=3.0)
+    assert st["ends"][arc.ARC_END_DEPLETED] > 0.5 * (st["ends"][1] + st["ends"][2])
+    assert_close(st["absorbed"] + st["escaped"], st["emitted"], 1e-10, "conservation with depletion")
+
+
+def test_config5_512_central_source_and_slab_chemistry():
+    w = wl.config5(N=512, nsrc=1024)
+    N = w.N
+    g = w.src_pos_cm / (w.box_cm / N)
+    s = int(np.argmin(np.sum((g - 0.5 * N) ** 2, axis=1)))       # the source nearest the centre: its rays cross half the box
+    assert np.all(np.abs(g[s] - 0.5 * N) < 0.2 * N)
+    Ao, so = oracle_trace_parallel(w, sources=np.array([s]), threads=8)
+    import torch
+    with arc.Context(w, digest=1) as cx:
+        cx.set_sources(np.array([s]))
+        cx.trace()
+        compare_trace_stats(cx.stats(), so, w.nb, R32)
+        A = torch.empty((w.ncell, w.nb), dtype=torch.float64, device="cuda")
+        arc.arc_get_accum(cx.ctx, A)
+        assert_close(A.cpu().numpy(), Ao, R32, "512^3 central source: A")
+        del A, Ao
+    # chemistry: all 1024 sources on the device, then the update of the slab iz in [240, 272) against the oracle
+    lo, hi = 240 * N * N, 272 * N * N
+    with arc.Context(w) as cx:
+        cx.trace()
+        rates = [torch.empty(w.ncell, dtype=torch.float64, device="cuda") for _ in range(6)]
+        arc.arc_get_rates(cx.ctx, *rates)
+        G = np.stack([r[lo:hi].cpu().numpy() for r in rates[:3]]); H = np.stack([r[lo:hi].cpu().numpy() for r in rates[3:]])
+        del rates
+        cx.update_chemistry()
+        got = [a[lo:hi] for a in cx.get_fields()]
+    before = [np.asarray(a)[lo:hi] for a in w.fields()]
+    want, sub = oracle_chemistry_parallel(w, before, G, H, w.dt_s)      # 2^23 cells, in chunks of 64^3
+    for name, a, b in zip(("x_HI", "x_HeI", "x_HeII", "T"), got[1:], want[1:]):
+        assert_close(a, b, R32, f"512^3 slab chemistry: {name}")
+    assert sub.max() > 1
+

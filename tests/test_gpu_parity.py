@@ -209,6 +209,55 @@ def test_api_error_behaviour():
         assert e.value.code == arc.ARC_EINVAL
 
 
+def test_source_that_rounds_onto_the_upper_face_is_rejected():
+    """with N not a power of two, pos just below box can give pos / (box / N) == N exactly: no cell.
+    Such a position is ARC_EINVAL; the nearest position that does have a cell traces like any other."""
+    N = 48
+    w = wl.tiny(N=N, nsrc=1, nb=1, seed=3, dtype="f64")
+    dx = w.box_cm / N
+    top = np.nextafter(w.box_cm, 0.0)
+    ctx = arc.arc_create_grid(N, w.box_cm, arc.ARC_F64)
+    try:
+        arc.arc_set_spectrum(ctx, w.E_eV, w.sig_HI, w.sig_HeI, w.sig_HeII)
+        x = top
+        rejected = 0
+        for _ in range(64):                               # walk down from the face until the quotient drops below N
+            pos = np.array([[x, 0.5 * w.box_cm, 0.5 * w.box_cm]])
+            if x / dx >= N:
+                with pytest.raises(arc.ArcError) as e:
+                    arc.arc_set_sources(ctx, pos, w.src_Ndot, w.src_binfrac)
+                assert e.value.code == arc.ARC_EINVAL
+                rejected += 1
+                x = np.nextafter(x, 0.0)
+            else:
+                arc.arc_set_sources(ctx, pos, w.src_Ndot, w.src_binfrac)
+                break
+        assert int(np.floor(x / dx)) == N - 1
+    finally:
+        arc.arc_destroy(ctx)
+    w.src_pos_cm = np.array([[x, 0.5 * w.box_cm, 0.5 * w.box_cm]])
+    (A, st, _), (Ao, so, _) = _trace_both(w)
+    compare_trace_stats(st, so, 1, RTOL["f64"])
+    assert_close(A, Ao, RTOL["f64"], "A (source in the last cell, next to the face)")
+
+
+def test_division_by_reciprocal_is_the_ieee_quotient():
+    """the identity the bit-exact traversal rests on (DESIGN.md 6.2 step 1, contract C3): 2^31 device-generated (a, d)
+    pairs in the ranges of the march, including divisors at and just below powers of two - not one differing bit"""
+    assert arc.arc_selftest_division(1 << 31, seed=180707094) == 0
+    assert arc.arc_selftest_division(1 << 24, seed=7) == 0
+    assert arc.arc_selftest_division(0) == 0
+
+
+def test_kernel_launches_are_counted():
+    w = wl.config1()
+    with arc.Context(w) as cx:
+        n0 = cx.stats()["kernel_launches"]
+        cx.trace(); cx.update_chemistry()
+        n1 = cx.stats()["kernel_launches"]
+    assert n0 == 0 and n1 == 5          # reset, opacity + zero, tracer, finalize, chemistry
+
+
 def test_ray_log_overflow_is_reported():
     w = wl.config1()
     with arc.Context(w) as cx:

@@ -220,3 +220,27 @@ def test_helium_iii_follows_the_hydrogenic_scaling():
             he = orc.rate_coeffs(4.0 * T, caseB=caseB)
             assert abs(he[2] / (2.0 * h[0]) - 1.0) < 2e-3
             assert abs(he[8] / (32.0 * h[6]) - 1.0) < 2e-3
+
+
+def test_update_is_ill_conditioned_where_the_limiter_switches():
+    """Evidence for how tests/test_gpu_chem.py compares whole steps (same rates on both sides, strict) - a property of the
+    paper's algorithm, shown on the oracle alone.  PAPER.md:152 sets the sub-step to min(eps E/|dE/dt|, eps n_HI/|dn_HI/dt|):
+    where heat - cool passes through zero the first bound jumps, the other takes over, and the first-order truncation
+    error of the step changes with it.  A 1e-7 relative change of the rates (a hundredth of the fp64 parity bar) then
+    moves some cells by > 1e-5 - an amplification of > 100 - although every cell takes the same number of sub-steps.
+    With an isothermal gas only the hydrogen bound is left (it jumps the same way where dn_HI/dt passes through zero,
+    near ionisation equilibrium) and the same perturbation is amplified five to ten times less."""
+    rng = np.random.default_rng(1)
+    amp = {}
+    for iso in (0, 1):
+        w = wl.tiny(N=12, nsrc=3, nb=3, seed=61, dtype="f64", Yp=0.24, kappa_scale=10.0)
+        w.params.update(isothermal=iso)
+        w.src_Ndot = w.src_Ndot * 1e3
+        ref = orc.step(w, w.fields())
+        G = ref["Gamma"] * (1 + 1e-7 * rng.uniform(-1, 1, ref["Gamma"].shape))
+        H = ref["heat"] * (1 + 1e-7 * rng.uniform(-1, 1, ref["heat"].shape))
+        f2, sub2 = orc.chemistry(w, w.fields(), G, H, w.dt_s)
+        assert np.array_equal(sub2, ref["subcycles"])                    # same sub-step counts everywhere
+        x1, x2 = ref["fields"][1], f2[1]
+        amp[iso] = float(np.max(np.abs(x1 - x2) / np.maximum(x1, x2))) / 1e-7
+    assert amp[0] > 100.0 and amp[1] < amp[0] / 5.0, amp
