@@ -13,6 +13,7 @@ fields below stand in for that workload's shape (DESIGN.md says so too).
 """
 from __future__ import annotations
 
+import functools
 from dataclasses import dataclass, field
 import numpy as np
 
@@ -129,14 +130,14 @@ def lognormal_density(N, rng, sigma_ln, mean=1e-3, kmax=None):
 
 
 def density_peaks(n3, count):
-    """Indices (iz,iy,ix) of the `count` highest 26-neighbour local maxima of n3[z,y,x]."""
+    """Cells (ix,iy,iz) and values of the `count` highest 26-neighbour local maxima of n3[z,y,x], highest first."""
     from scipy.ndimage import maximum_filter
     mx = maximum_filter(n3, size=3, mode="nearest")
     cand = np.flatnonzero((n3 == mx).ravel())
     vals = n3.ravel()[cand]
-    order = np.argsort(-vals, kind="stable")[:count]
+    order = np.argsort(-vals, kind="stable")[:count]          # (count = None: all of them)
     idx = cand[order]
-    if idx.size < count:
+    if count is not None and idx.size < count:
         raise ValueError(f"only {idx.size} local maxima, need {count}")
     iz, iy, ix = np.unravel_index(idx, n3.shape)
     return np.stack([ix, iy, iz], axis=1), vals[order]
@@ -218,11 +219,24 @@ def config3(N=128, nsrc=16, dtype="f64"):
     return w
 
 
-def _peaks_workload(name, N, nsrc, sigma_ln, seed, n_steps, kmax=None, state="neutral"):
+@functools.lru_cache(maxsize=2)
+def _peaks_field(N, sigma_ln, seed, kmax):
+    """the density field of configs 4 / 5 and its local maxima in decreasing order (cached: a source-count sweep on one
+    grid shares them; the 512^3 field takes half a minute to make)"""
     rng = np.random.default_rng(seed)
-    box = 15.0 * KPC_CM
     n3 = _clumpy(N, rng, sigma_ln, kmax=kmax)
-    pk, vals = density_peaks(n3, nsrc)
+    pk, vals = density_peaks(n3, None)
+    for a in (n3, pk, vals):
+        a.setflags(write=False)
+    return n3, pk, vals
+
+
+def _peaks_workload(name, N, nsrc, sigma_ln, seed, n_steps, kmax=None, state="neutral"):
+    box = 15.0 * KPC_CM
+    n3, pk, vals = _peaks_field(N, sigma_ln, seed, kmax)
+    if len(vals) < nsrc:
+        raise ValueError(f"only {len(vals)} local maxima, need {nsrc}")
+    pk, vals = pk[:nsrc].copy(), vals[:nsrc].copy()
     Ndot = 1e48 * vals / vals.mean()
     E, s1, s2, s3, frac = powerlaw_spectrum([E_HI, E_HEI, E_HEII, 100.0, 200.0])
     n = N ** 3

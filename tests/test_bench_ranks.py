@@ -65,6 +65,33 @@ def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
     assert d["config"]["workload"] == "config1" and d["value"] > 0
 
 
+def test_gpus_flag_starts_its_own_ranks_without_torchrun():
+    """`python bench.py --gpus 2` with no torchrun environment (how the driver calls it at N = 1) must start two ranks
+    itself: one JSON line from rank 0 with n_gpus = 2, and rank 1 was really there"""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+                        "--warmup", "0", "--config", "config1"], capture_output=True, text=True, cwd=ROOT, timeout=600, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
+    assert "rank 1 of 2" in r.stderr
+
+
+def test_bench_defaults_to_the_largest_single_gpu_configuration():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.DEFAULT_CONFIG == "config5_N512_S1024"
+    names = [n for n, _, _ in bench.PER_CONFIG]
+    assert names[:4] == ["config1", "config2", "config3", "config4"] and all(n.startswith("config5_N") for n in names[4:])
+    # a committed ncu capture is only used for the workload, flags and csrc build it was taken on
+    cap, why = bench.ncu_capture("config5_N512_S1024", 1.0, {"geom_corr": 0})
+    assert cap is None and "different number of segments" in why or "no committed" in why or "another build" in why
+    cap, why = bench.ncu_capture("config4", 1.0, {"geom_corr": 2})
+    assert cap is None
+
+
 def test_cuda_arm_refuses_to_run_without_a_device():
     if torch.cuda.is_available():
         return

@@ -5,7 +5,7 @@ Configs 4 and 5 are out of the oracle's reach in full (1e11-1e12 segments per st
     fields a free-running device run has reached at steps 0, 10 and 19 - injected into both sides;
   * the CHEMISTRY is compared on the whole 256^3 fp32 grid (every cell, strict) with the device's own rates of those
     steps handed to the oracle - the first comparison of arc_chem_kernel<float> at the size the bench runs;
-  * one full-size fp32 case ends rays DEPLETED (tau_term = 3), which config 4 as specified never does;
+  * one full-size fp32 case ends rays DEPLETED (tau_term = 0.5), which config 4 as specified never does;
   * config 5: the source nearest the centre of the 512^3 grid, and the chemistry on a 512 x 512 x 32 slab.
 The oracle runs on all host cores here (gpu_common.oracle_*_parallel: the unchanged single-threaded C routine, called on
 disjoint shares of the rays / cells); bench.py times it as it stands.
@@ -77,14 +77,14 @@ def test_config4_sixteen_sources_and_the_whole_grid_chemistry_at_steps_0_10_19()
 
 
 def test_config4_sixteen_sources_with_rays_that_deplete():
-    """tau_term = 3 on the neutral step-0 fields: most rays end DEPLETED a few cells from their source (config 4 as
-    specified never gets there: its hardest bin stays below tau_term = 30) - the depleted branch of
-    arc_trace_kernel<4, float> at full size"""
+    """tau_term = 0.5 on the neutral step-0 fields: a third of the rays end DEPLETED on their way through the box (config 4
+    as specified never gets there: the optical depth of its hardest bin across the box stays below 2, far from
+    tau_term = 30) - the depleted branch of arc_trace_kernel<4, float> at full size"""
     w = wl.config4()
     rng = np.random.default_rng(wl.SEED0 + 417)
     sample = np.sort(rng.choice(w.nsrc, size=16, replace=False))
-    st = _subset_parity(w, w.fields(), sample, "tau_term = 3", tau_term=3.0)
-    assert st["ends"][arc.ARC_END_DEPLETED] > 0.5 * (st["ends"][1] + st["ends"][2])
+    st = _subset_parity(w, w.fields(), sample, "tau_term = 0.5", tau_term=0.5)
+    assert st["ends"][arc.ARC_END_DEPLETED] > 0.25 * (st["ends"][1] + st["ends"][2])
     assert_close(st["absorbed"] + st["escaped"], st["emitted"], 1e-10, "conservation with depletion")
 
 
