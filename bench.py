@@ -181,7 +181,7 @@ def oracle_trace_sample(w, budget_s=12.0, units=None):
         seg, secs, A = run(u)
         if secs >= budget_s / 2.0 or u >= total:
             return seg, secs, u, A
-        u = int(min(total, max(u + 1, u * min(16.0, 0.8 * budget_s / max(secs, 1e-3)))))
+        u = int(min(total, max(u + 1, u * min(4.0, 0.6 * budget_s / max(secs, 1e-3)))))
 
 
 def sample_text(w, units):
@@ -284,7 +284,7 @@ def self_launch(argv, n: int) -> int:
 
 
 # ------------------------------------------------------------------------------------------------ CUDA arm
-def timed_run(w, steps, warmup, extra, stream, shard_sources=None, barrier=None, sampler_index=None):
+def timed_run(w, steps, warmup, extra, stream, shard_sources=None, barrier=None, sampler_index=None, graph_steps=0):
     """`warmup` untimed + `steps` timed steps with the fields resident in HBM; device times from CUDA events on the
     library's stream.  -> dict of raw measurements of THIS rank."""
     import torch
@@ -333,6 +333,17 @@ def timed_run(w, steps, warmup, extra, stream, shard_sources=None, barrier=None,
     out["launches"] = cons["kernel_launches"] - launches0
     out["stats"] = cons
     out["trace_grid"] = cons["trace_grid"]
+    if graph_steps:
+        # the same loop through arc_run_steps: one captured CUDA graph per step, replayed, one synchronisation at the end
+        cx.set_fields(dev_fields)                 # (from the initial fields again)
+        cx.run_steps(max(3, warmup))
+        s0 = cx.stats()
+        cx.run_steps(graph_steps)
+        s1 = cx.stats()
+        seg = s1["segments_total"] - s0["segments_total"]
+        out["graph"] = {"steps": graph_steps, "ms_per_step": s1["steps_ms"] / graph_steps,
+                        "segments_per_s": seg / (s1["steps_ms"] * 1e-3) if s1["steps_ms"] > 0 else 0.0,
+                        "launches_per_step": (s1["kernel_launches"] - s0["kernel_launches"]) / graph_steps}
     cx.close()
     del dev_fields
     return out
@@ -495,9 +506,11 @@ def run_cuda(args):
                     continue
                 wc = make_workload(name)
                 with torch.cuda.stream(stream):
-                    rc = timed_run(wc, k, wu, {}, stream)
+                    rc = timed_run(wc, k, wu, {}, stream, graph_steps=(10 * k if wc.nsrc <= 16 else 0))
                 per[wc.name] = dict(summarise(wc, rc, k, peak), warmup=wu, steps=k,
                                     **{kk: describe(wc)[kk] for kk in ("grid", "sources", "freq_bins", "field_dtype")})
+                if "graph" in rc:
+                    per[wc.name]["arc_run_steps"] = rc["graph"]
                 del wc, rc
             line["per_config"] = per
         if world == 1 and not args.no_cpu_baseline:

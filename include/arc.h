@@ -115,6 +115,11 @@ typedef struct arc_stats {
     uint64_t deposit_records;          /* accumulator records sent to L2 (<= segments: warp-aggregated deposit) */
     uint64_t kernel_launches;          /* kernels this context has launched since arc_create_grid (counted on the host at
                                           every launch of the library's own kernels; memsets and copies are not kernels) */
+    uint64_t segments_total;           /* segments / chemistry sub-cycles of ALL traces / updates since arc_create_grid    */
+    uint64_t subcycles_total;          /*   (the per-call counters above are those of the last call only)                 */
+    float    steps_ms;                 /* arc_run_steps: CUDA-event duration of all its steps together (the per-kernel times
+                                          above are then 0: events cannot be timed inside a captured graph)             */
+    int32_t  pad3;
 } arc_stats;
 
 /* Caller-provided HOST buffers for arc_trace_debug: one entry per segment (seq = 0,1,2,... within the
@@ -193,6 +198,16 @@ int arc_get_accum(arc_ctx *c, double *A, int where);
  * last arc_trace held fixed (PAPER.md:57 step v; :136-154 Eq. 4-5; :166-172).  ARC_ESTATE if no
  * trace has been done since the fields were last set. */
 int arc_update_chemistry(arc_ctx *c, double dt_s);
+
+/* The time-step loop of PAPER.md:47-59 (steps i, iii, v, vii) without a host round trip per step: n_steps times
+ * { arc_trace; arc_update_chemistry(dt_s) }, enqueued back to back - one step is captured once into a CUDA graph (opacity +
+ * reset, tracer, finalize, chemistry) and replayed - then ONE synchronisation and error check (none with async = 1).
+ * The fields advance n_steps x dt_s; rates and per-call statistics are those of the last step, segments_total /
+ * subcycles_total count all of them, steps_ms times them together.  Small grids, where launches and synchronisation cost
+ * more than the kernels, are what this is for.  Needs a stream set with arc_set_stream for the graph
+ * (on the legacy default stream the steps are enqueued one by one instead).  Errors as arc_trace; ARC_EINVAL with
+ * thin_tau > 0 (each of those traces hands its radii to the host). */
+int arc_run_steps(arc_ctx *c, int n_steps, double dt_s);
 
 /* Anisotropic emission: blocked[s * npix0 + p] != 0 blocks root ray p (nested pixel of level l0,
  * npix0 = 12 * 4^l0) of source s: it does not exist - no packet, no segments, not in `emitted`; the open rays carry the

@@ -30,7 +30,7 @@ LIB_PATH = os.path.join(_HERE, "libarc_b200.so")
 EXPORTS = ["arc_create_grid", "arc_destroy", "arc_default_params", "arc_set_params", "arc_set_stream",
            "arc_set_fields", "arc_get_fields", "arc_set_spectrum", "arc_set_sources", "arc_set_emission_mask", "arc_get_thin_radii", "arc_set_thin_radii", "arc_trace",
            "arc_trace_partial", "arc_accum_device", "arc_finalize",
-           "arc_get_rates", "arc_get_accum", "arc_update_chemistry", "arc_suggest_dt", "arc_synchronize", "arc_get_stats",
+           "arc_get_rates", "arc_get_accum", "arc_update_chemistry", "arc_run_steps", "arc_suggest_dt", "arc_synchronize", "arc_get_stats",
            "arc_trace_debug", "arc_pix2vec", "arc_selftest_division", "arc_last_error", "arc_version"]
 
 
@@ -62,7 +62,8 @@ class arc_stats(C.Structure):
                 ("max_subcycles_cell", C.c_uint32), ("pad", C.c_uint32), ("trace_ms", C.c_float),
                 ("chem_ms", C.c_float), ("trace_kernel_ms", C.c_float), ("opacity_ms", C.c_float),
                 ("finalize_ms", C.c_float), ("trace_grid", C.c_int32), ("pad2", C.c_int32),
-                ("deposit_records", C.c_uint64), ("kernel_launches", C.c_uint64)]
+                ("deposit_records", C.c_uint64), ("kernel_launches", C.c_uint64), ("segments_total", C.c_uint64),
+                ("subcycles_total", C.c_uint64), ("steps_ms", C.c_float), ("pad3", C.c_int32)]
 
 
 class arc_raylog(C.Structure):
@@ -98,6 +99,7 @@ def lib():
         l.arc_finalize.argtypes = [vp, C.POINTER(arc_rates)]
         l.arc_get_accum.argtypes = [vp, vp, i32]
         l.arc_update_chemistry.argtypes = [vp, dbl]
+        l.arc_run_steps.argtypes = [vp, i32, dbl]
         l.arc_suggest_dt.argtypes = [vp, i32, dbl, vp, vp]
         l.arc_set_emission_mask.argtypes = [vp, vp, i32]
         l.arc_get_thin_radii.argtypes = [vp, vp]
@@ -248,6 +250,11 @@ def arc_update_chemistry(ctx, dt_s: float):
     return _check(ctx, lib().arc_update_chemistry(ctx, float(dt_s)))
 
 
+def arc_run_steps(ctx, n_steps: int, dt_s: float):
+    """n_steps x (arc_trace + arc_update_chemistry(dt_s)) without a host round trip per step (one CUDA graph, replayed)"""
+    return _check(ctx, lib().arc_run_steps(ctx, int(n_steps), float(dt_s)))
+
+
 ARC_DT_NEUTRAL, ARC_DT_INTENSITY = 1, 2
 
 
@@ -328,7 +335,8 @@ def stats_dict(s: arc_stats, nb: int) -> dict:
                 subcycles=int(s.subcycles), max_subcycles_cell=int(s.max_subcycles_cell),
                 trace_ms=float(s.trace_ms), chem_ms=float(s.chem_ms), trace_kernel_ms=float(s.trace_kernel_ms),
                 opacity_ms=float(s.opacity_ms), finalize_ms=float(s.finalize_ms), trace_grid=int(s.trace_grid),
-                deposit_records=int(s.deposit_records), kernel_launches=int(s.kernel_launches))
+                deposit_records=int(s.deposit_records), kernel_launches=int(s.kernel_launches),
+                segments_total=int(s.segments_total), subcycles_total=int(s.subcycles_total), steps_ms=float(s.steps_ms))
 
 
 def params_from_dict(d: dict, **override) -> arc_params:
@@ -433,6 +441,9 @@ class Context:
 
     def update_chemistry(self, dt=None):
         return arc_update_chemistry(self.ctx, self.w.dt_s if dt is None else dt)
+
+    def run_steps(self, n_steps, dt=None):
+        return arc_run_steps(self.ctx, n_steps, self.w.dt_s if dt is None else dt)
 
     def stats(self):
         return stats_dict(arc_get_stats(self.ctx), self.nb)

@@ -97,6 +97,8 @@ int arc_destroy(arc_ctx *c)
     cudaFree(c->d_kappa); cudaFree(c->d_A); cudaFree(c->d_src_g); cudaFree(c->d_src_S);
     cudaFree(c->d_stacks); cudaFree(c->d_queue); cudaFree(c->d_qseq);
     for (int i = 0; i < 8; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    for (int i = 0; i < 2; ++i) if (c->ev_steps[i]) cudaEventDestroy(c->ev_steps[i]);
+    if (c->step_exec) cudaGraphExecDestroy(c->step_exec);
     delete c;
     return ARC_OK;
 }
@@ -122,7 +124,7 @@ int arc_set_params(arc_ctx *c, const arc_params *p)
     if (p->geom_corr != ARC_GEOM_NONE && p->deposit != ARC_DEPOSIT_AUTO)
         return fail(c, ARC_EINVAL, "arc_set_params: the geometric correction is built for deposit = ARC_DEPOSIT_AUTO only");
     c->p = *p;
-    c->have_rates = false; c->have_accum = false;
+    c->have_rates = false; c->have_accum = false; ++c->epoch;
     return ARC_OK;
 }
 
@@ -130,7 +132,7 @@ int arc_set_stream(arc_ctx *c, void *cuda_stream)
 {
     if (!c) return ARC_EINVAL;
     cudaStreamSynchronize(c->stream);
-    c->stream = (cudaStream_t)cuda_stream;
+    c->stream = (cudaStream_t)cuda_stream; ++c->epoch;
     return ARC_OK;
 }
 
@@ -185,7 +187,7 @@ int arc_set_spectrum(arc_ctx *c, int nbins, const double *E_eV, const double *si
         c->spec.E[v] = E_eV[v]; c->spec.sig[0][v] = sig_HI[v]; c->spec.sig[1][v] = sig_HeI[v]; c->spec.sig[2][v] = sig_HeII[v];
     }
     c->have_spec = true;
-    c->have_rates = false; c->have_accum = false;
+    c->have_rates = false; c->have_accum = false; ++c->epoch;
     return ARC_OK;
 }
 
@@ -228,7 +230,7 @@ int arc_set_sources(arc_ctx *c, int nsrc, const double *pos_cm, const double *Nd
     }
     c->nsrc = nsrc;
     c->have_src = true;
-    c->have_rates = false; c->have_accum = false;
+    c->have_rates = false; c->have_accum = false; ++c->epoch;
     return ARC_OK;
 }
 
@@ -261,6 +263,7 @@ int arc_set_emission_mask(arc_ctx *c, const uint8_t *blocked, int level)
     CK(cudaStreamSynchronize(c->stream));
     cudaFree(c->d_blocked); c->d_blocked = nullptr; c->mask_level = -1;
     for (int v = 0; v < ARC_MAX_BINS; ++v) c->emitted[v] = 0.0;
+    ++c->epoch;
     if (!blocked) {
         c->h_nopen.assign((size_t)c->nsrc, -1.0);
         for (int s = 0; s < c->nsrc; ++s) for (int v = 0; v < nb; ++v) c->emitted[v] += c->h_src_S[(size_t)s * nb + v];

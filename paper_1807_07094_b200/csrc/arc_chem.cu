@@ -203,7 +203,7 @@ __global__ void __launch_bounds__(128) arc_chem_iso_kernel(long long ncell, doub
         my_sub += __shfl_xor_sync(0xffffffffu, my_sub, o);
         my_max = max(my_max, __shfl_xor_sync(0xffffffffu, my_max, o));
     }
-    if ((threadIdx.x & 31) == 0) { atomicAdd(&stats->subcycles, my_sub); atomicMax(&stats->max_sub, my_max); }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&stats->subcycles, my_sub); atomicAdd(&stats->subcycles_total, my_sub); atomicMax(&stats->max_sub, my_max); }
 }
 
 // Evolving temperature: every sub-cycle re-evaluates the rate table (a few thousand fp64 instructions) and the number of
@@ -256,7 +256,7 @@ __global__ void __launch_bounds__(128, 5) arc_chem_kernel(long long ncell, doubl
         my_sub += __shfl_xor_sync(0xffffffffu, my_sub, o);
         my_max = max(my_max, __shfl_xor_sync(0xffffffffu, my_max, o));
     }
-    if (lane == 0) { atomicAdd(&stats->subcycles, my_sub); atomicMax(&stats->max_sub, my_max); }
+    if (lane == 0) { atomicAdd(&stats->subcycles, my_sub); atomicAdd(&stats->subcycles_total, my_sub); atomicMax(&stats->max_sub, my_max); }
 }
 
 // Radiative-transfer time step (include/arc.h arc_suggest_dt): one streaming pass, 28 B per cell

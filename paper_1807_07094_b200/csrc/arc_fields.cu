@@ -15,8 +15,21 @@ template <typename FT>
 __global__ void __launch_bounds__(256) arc_opacity_kernel(long long ncell, int nb, int nbp, double Yp, Spectrum sp,
                                                          const FT *__restrict__ nH, const FT *__restrict__ xHI,
                                                          const FT *__restrict__ xHeI, const FT *__restrict__ xHeII,
-                                                         FT *__restrict__ kappa, double *__restrict__ A)
+                                                         FT *__restrict__ kappa, double *__restrict__ A,
+                                                         SchedState *sc, DevStats *st, double *absorbed, unsigned long long seed_total, int fault)
 {
+    // per-trace reset of the scheduler words and tallies (the tracer is the next kernel on the stream): all root families
+    // are "in flight".  The error word is STICKY: what an earlier asynchronous trace left behind, and the host has not yet
+    // seen and cleared (arc_check_device), stays - the tracer then does not run and every consumer kernel keeps skipping.
+    // `fault` = arc_params.debug_fault (test hook).
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        sc->in_flight = (long long)seed_total; sc->seed_next = 0; sc->hungry = 0; sc->q_high = 0; sc->log_n = 0;
+        if (sc->error == ARC_DEV_OK) sc->error = fault;
+        st->segments = 0; st->rays = 0; st->digest = 0; st->deposit_records = 0;
+        for (int l = 0; l < ARC_MAX_LEVEL; ++l) { st->splits[l] = 0; st->rays_level[l] = 0; }
+        for (int e = 0; e < 3; ++e) st->ends[e] = 0;
+        for (int v = 0; v < ARC_MAX_BINS; ++v) { st->escaped[v] = 0.0; absorbed[v] = 0.0; }
+    }
     for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
         const double n = (double)nH[c];
         const double nHe = n_helium(n, Yp);
@@ -98,17 +111,17 @@ static int stream_grid(arc_ctx *c, long long n)
     return (int)(b < cap ? b : cap);
 }
 
-cudaError_t arc_launch_opacity(arc_ctx *c)
+cudaError_t arc_launch_opacity(arc_ctx *c, unsigned long long seed_total)
 {
     const int g = stream_grid(c, c->ncell);
     if (c->dtype == ARC_F32)
         arc_opacity_kernel<float><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, arc_nbp(c->spec.nb), c->p.Yp, c->spec, (const float *)c->f[0],
                                                           (const float *)c->f[1], (const float *)c->f[2], (const float *)c->f[3],
-                                                          (float *)c->d_kappa, c->d_A);
+                                                          (float *)c->d_kappa, c->d_A, c->d_sched, c->d_stats, c->d_absorbed, seed_total, c->p.debug_fault);
     else
         arc_opacity_kernel<double><<<g, 256, 0, c->stream>>>(c->ncell, c->spec.nb, arc_nbp(c->spec.nb), c->p.Yp, c->spec, (const double *)c->f[0],
                                                            (const double *)c->f[1], (const double *)c->f[2], (const double *)c->f[3],
-                                                           (double *)c->d_kappa, c->d_A);
+                                                           (double *)c->d_kappa, c->d_A, c->d_sched, c->d_stats, c->d_absorbed, seed_total, c->p.debug_fault);
     ++c->launches;
     return cudaGetLastError();
 }
@@ -167,8 +180,6 @@ cudaError_t arc_launch_thin_region(arc_ctx *c, double maxR)
 
 cudaError_t arc_launch_finalize(arc_ctx *c)
 {
-    cudaError_t e = cudaMemsetAsync(c->d_absorbed, 0, sizeof(double) * ARC_MAX_BINS, c->stream);
-    if (e != cudaSuccess) return e;
     const int g = stream_grid(c, c->ncell);
     const double V = c->dx * c->dx * c->dx;
     if (c->dtype == ARC_F32)

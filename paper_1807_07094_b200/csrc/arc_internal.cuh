@@ -51,6 +51,7 @@ struct SchedState {
 };
 
 struct DevStats {
+    unsigned long long segments_total, subcycles_total;     // since arc_create_grid: never reset (arc_run_steps reads them once)
     unsigned long long segments, rays, digest, deposit_records;
     unsigned long long splits[ARC_MAX_LEVEL];
     unsigned long long rays_level[ARC_MAX_LEVEL];
@@ -141,16 +142,21 @@ struct arc_ctx {
     bool have_accum = false;          // arc_trace_partial ran: the accumulators wait for arc_finalize
     bool finalize_split = false;      // the last finalise pass was arc_finalize's (events 4, 7)
     unsigned long long launches = 0;  // kernels launched by this context (arc_stats.kernel_launches)
+    bool queue_dirty = true;          // the donation queue needs its full reset (first trace, or the last one aborted)
+    unsigned long long epoch = 0;     // bumped by every call that changes what a captured step graph bakes in
+    cudaGraphExec_t step_exec = nullptr; unsigned long long step_epoch = 0; double step_dt = 0.0;   // arc_run_steps
+    unsigned long long step_launches = 0;    // kernels in one replay of that graph
+    cudaEvent_t ev_steps[2] = {nullptr, nullptr}; bool steps_timed = false;
     bool unchecked = false;           // an asynchronous trace has been enqueued and its device error word not yet looked at
     std::string err;
 };
 
 // arc_fields.cu
-cudaError_t arc_launch_opacity(arc_ctx *c);
+cudaError_t arc_launch_opacity(arc_ctx *c, unsigned long long seed_total);    // a1 + a2 + the per-trace scheduler / tally reset
 cudaError_t arc_launch_finalize(arc_ctx *c);
 cudaError_t arc_launch_thin_region(arc_ctx *c, double maxR);     // inner-region deposit for the sources with Rstart > 0
 // arc_trace.cu
-cudaError_t arc_launch_sched_reset(arc_ctx *c, unsigned long long seed_total);
+cudaError_t arc_launch_queue_reset(arc_ctx *c);        // full reset of the donation queue (first trace / after an aborted one)
 cudaError_t arc_launch_trace(arc_ctx *c, const TraceArgs &a, bool log, int *grid_out);
 int arc_trace_occupancy_grid(arc_ctx *c, int nb, int flags);   // flags: 1 log, 2 digest
 cudaError_t arc_launch_pix2vec(const int32_t *d_level, const uint32_t *d_pix, int n, double *d_out, cudaStream_t s);

@@ -29,6 +29,7 @@ int arc_check_device(arc_ctx *c)
     CK(cudaMemcpy(&h, c->d_sched, sizeof(h), cudaMemcpyDeviceToHost));
     if (h.error == ARC_DEV_OK && h.in_flight == 0) return ARC_OK;
     c->have_rates = false; c->have_accum = false;
+    c->queue_dirty = true;                        // families may be left in the donation queue: full reset before the next trace
     CK(cudaMemset(&c->d_sched->error, 0, sizeof(int)));
     switch (h.error) {
         case ARC_DEV_STACK_OVERFLOW: return fail(c, ARC_EOVERFLOW, "arc_trace: a warp's work stack overflowed; rates are invalid");
@@ -39,7 +40,9 @@ int arc_check_device(arc_ctx *c)
     }
 }
 
-static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, unsigned int *d_seq, int *d_cell, bool finalize = true)
+// host side of a trace: state checks, (re)allocation of the work stacks and the queue, the kernel's arguments, and - with
+// an optically thin region - the per-source start radii.  Nothing is enqueued except those small copies.
+static int prepare_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, unsigned int *d_seq, int *d_cell, TraceArgs &a, double &thin_maxR)
 {
     if (!c->have_fields) return fail(c, ARC_ESTATE, "arc_trace: no fields set (arc_set_fields)");
     if (!c->have_spec) return fail(c, ARC_ESTATE, "arc_trace: no spectrum set (arc_set_spectrum)");
@@ -62,17 +65,16 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
         CK(cudaStreamSynchronize(c->stream));
         cudaFree(c->d_stacks); c->d_stacks = nullptr; c->stacks_bytes = 0;
         CK(cudaMalloc(&c->d_stacks, need_stacks));
-        c->stacks_bytes = need_stacks;
+        c->stacks_bytes = need_stacks; ++c->epoch;
     }
     if (need_queue > c->queue_bytes) {
         CK(cudaStreamSynchronize(c->stream));
         cudaFree(c->d_queue); c->d_queue = nullptr; c->queue_bytes = 0;
         CK(cudaMalloc(&c->d_queue, need_queue));
-        c->queue_bytes = need_queue;
+        c->queue_bytes = need_queue; ++c->epoch;
     }
-    if (!c->d_qseq) CK(cudaMalloc(&c->d_qseq, sizeof(unsigned long long) * ARC_QUEUE_CAP));
+    if (!c->d_qseq) { CK(cudaMalloc(&c->d_qseq, sizeof(unsigned long long) * ARC_QUEUE_CAP)); c->queue_dirty = true; }
 
-    TraceArgs a;
     std::memset(&a, 0, sizeof(a));
     a.N = c->N; a.NN = c->N * c->N; a.max_seg = 3u * (unsigned)c->N + 8u; a.nb = nb; a.nbp = arc_nbp(nb); a.l0 = c->p.l0; a.Lmax = c->p.Lmax; a.nsrc = c->nsrc;
     a.dx = c->dx;
@@ -84,7 +86,7 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
     a.stacks = c->d_stacks; a.queue = c->d_queue; a.qseq = c->d_qseq; a.sched = c->d_sched; a.stats = c->d_stats;
     a.fam_per_src = 3u << (2 * c->p.l0);
     a.seed_total = (unsigned long long)c->nsrc * a.fam_per_src;
-    double thin_maxR = 0.0;
+    thin_maxR = 0.0;
     if (thin && c->nsrc > 0) {
         // optically thin inner region: per source, the radius the last trace found, the level rays have
         // there (r_split(l-1) <= R < r_split(l)), its root families, and the rate the open root rays carry together
@@ -130,17 +132,32 @@ static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, uns
     }
     a.flags = flags;
     a.log_key = d_key; a.log_seq = d_seq; a.log_cell = d_cell; a.log_cap = log ? (unsigned long long)log->cap : 0ull;
+    return ARC_OK;
+}
 
-    CK(cudaEventRecord(c->ev[0], c->stream));
-    CK(arc_launch_sched_reset(c, a.seed_total));
-    CK(arc_launch_opacity(c));
-    if (thin && thin_maxR > 0.0) CK(arc_launch_thin_region(c, thin_maxR));          // (iii): after the accumulators are zeroed
-    CK(cudaEventRecord(c->ev[1], c->stream));
-    CK(arc_launch_trace(c, a, log != nullptr, nullptr));
-    CK(cudaEventRecord(c->ev[2], c->stream));
+// the kernels of one trace, in stream order: [queue reset if needed] -> a1 + a2 + per-trace reset -> [thin region] ->
+// a3-a9 persistent tracer -> a10 finalize.  `events`: bracket them with the context's CUDA events (not inside a graph capture).
+static int enqueue_trace(arc_ctx *c, const TraceArgs &a, bool log, bool finalize, double thin_maxR, bool events)
+{
+    if (c->queue_dirty) { CK(arc_launch_queue_reset(c)); c->queue_dirty = false; }
+    if (events) CK(cudaEventRecord(c->ev[0], c->stream));
+    CK(arc_launch_opacity(c, a.seed_total));
+    if (thin_maxR > 0.0) CK(arc_launch_thin_region(c, thin_maxR));          // (iii): after the accumulators are zeroed
+    if (events) CK(cudaEventRecord(c->ev[1], c->stream));
+    CK(arc_launch_trace(c, a, log, nullptr));
+    if (events) CK(cudaEventRecord(c->ev[2], c->stream));
     if (finalize) CK(arc_launch_finalize(c));          // arc_trace_partial leaves a10 to arc_finalize
-    CK(cudaEventRecord(c->ev[3], c->stream));
-    c->traced_once = true;
+    if (events) CK(cudaEventRecord(c->ev[3], c->stream));
+    return ARC_OK;
+}
+
+static int run_trace(arc_ctx *c, arc_raylog *log, unsigned long long *d_key, unsigned int *d_seq, int *d_cell, bool finalize = true)
+{
+    TraceArgs a; double thin_maxR = 0.0;
+    { const int rc = prepare_trace(c, log, d_key, d_seq, d_cell, a, thin_maxR); if (rc != ARC_OK) return rc; }
+    const bool thin = c->p.thin_tau > 0.0;
+    { const int rc = enqueue_trace(c, a, log != nullptr, finalize, thin ? thin_maxR : 0.0, true); if (rc != ARC_OK) return rc; }
+    c->traced_once = true; c->steps_timed = false;
     c->have_rates = finalize;
     c->have_accum = !finalize;
     c->finalize_split = false;
@@ -275,15 +292,66 @@ int arc_get_accum(arc_ctx *c, double *A, int where)
     return ARC_OK;
 }
 
+static int enqueue_chemistry(arc_ctx *c, double dt_s, bool events)
+{
+    if (events) CK(cudaEventRecord(c->ev[5], c->stream));
+    CK(cudaMemsetAsync(&c->d_stats->subcycles, 0, 2 * sizeof(unsigned long long) + 2 * sizeof(unsigned int), c->stream));
+    CK(arc_launch_chemistry(c, dt_s));
+    if (events) CK(cudaEventRecord(c->ev[6], c->stream));
+    return ARC_OK;
+}
+
+int arc_run_steps(arc_ctx *c, int n_steps, double dt_s)
+{
+    if (!c) return ARC_EINVAL;
+    if (n_steps < 1) return fail(c, ARC_EINVAL, "arc_run_steps: n_steps must be >= 1");
+    if (!(dt_s >= 0.0) || !std::isfinite(dt_s)) return fail(c, ARC_EINVAL, "arc_run_steps: dt must be finite and >= 0");
+    if (c->p.thin_tau > 0.0) return fail(c, ARC_EINVAL, "arc_run_steps: not built for thin_tau > 0 (every trace hands its radii to the host)");
+    TraceArgs a; double thin_maxR = 0.0;
+    { const int rc = prepare_trace(c, nullptr, nullptr, nullptr, nullptr, a, thin_maxR); if (rc != ARC_OK) return rc; }
+    if (!c->ev_steps[0]) { CK(cudaEventCreate(&c->ev_steps[0])); CK(cudaEventCreate(&c->ev_steps[1])); }
+    if (c->queue_dirty) { CK(arc_launch_queue_reset(c)); c->queue_dirty = false; }
+    // one step = the kernels of arc_trace + arc_update_chemistry; captured once into a CUDA graph (a user stream is needed:
+    // the legacy default stream cannot be captured - the steps are then enqueued one by one, still without a host round trip)
+    const bool use_graph = c->stream != nullptr;
+    if (use_graph && (!c->step_exec || c->step_epoch != c->epoch || c->step_dt != dt_s)) {
+        if (c->step_exec) { cudaGraphExecDestroy(c->step_exec); c->step_exec = nullptr; }
+        cudaGraph_t g = nullptr;
+        const unsigned long long l0 = c->launches;
+        CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+        int rc = enqueue_trace(c, a, false, true, 0.0, false);
+        if (rc == ARC_OK) rc = enqueue_chemistry(c, dt_s, false);
+        const cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+        if (rc != ARC_OK || e != cudaSuccess) { if (g) cudaGraphDestroy(g); cudaGetLastError(); return rc != ARC_OK ? rc : fail(c, ARC_ECUDA, std::string("arc_run_steps: graph capture: ") + cudaGetErrorString(e)); }
+        c->step_launches = c->launches - l0; c->launches = l0;        // (captured, not launched)
+        const cudaError_t e2 = cudaGraphInstantiate(&c->step_exec, g, 0);
+        cudaGraphDestroy(g);
+        if (e2 != cudaSuccess) { c->step_exec = nullptr; return fail(c, ARC_ECUDA, std::string("arc_run_steps: cudaGraphInstantiate: ") + cudaGetErrorString(e2)); }
+        c->step_epoch = c->epoch; c->step_dt = dt_s;
+    }
+    CK(cudaEventRecord(c->ev_steps[0], c->stream));
+    for (int i = 0; i < n_steps; ++i) {
+        if (use_graph) { CK(cudaGraphLaunch(c->step_exec, c->stream)); c->launches += c->step_launches; }
+        else {
+            int rc = enqueue_trace(c, a, false, true, 0.0, false);
+            if (rc == ARC_OK) rc = enqueue_chemistry(c, dt_s, false);
+            if (rc != ARC_OK) return rc;
+        }
+    }
+    CK(cudaEventRecord(c->ev_steps[1], c->stream));
+    c->traced_once = true; c->chem_once = true; c->steps_timed = true;
+    c->have_rates = true; c->have_accum = false; c->finalize_split = false;
+    if (!c->p.async) { CK(cudaStreamSynchronize(c->stream)); return arc_check_device(c); }
+    c->unchecked = true;
+    return ARC_OK;
+}
+
 int arc_update_chemistry(arc_ctx *c, double dt_s)
 {
     if (!c) return ARC_EINVAL;
     if (!(dt_s >= 0.0) || !std::isfinite(dt_s)) return fail(c, ARC_EINVAL, "arc_update_chemistry: dt must be finite and >= 0");
     if (!c->have_rates) return fail(c, ARC_ESTATE, "arc_update_chemistry: no valid rates (call arc_trace after setting fields)");
-    CK(cudaEventRecord(c->ev[5], c->stream));
-    CK(cudaMemsetAsync(&c->d_stats->subcycles, 0, 2 * sizeof(unsigned long long) + 2 * sizeof(unsigned int), c->stream));
-    CK(arc_launch_chemistry(c, dt_s));
-    CK(cudaEventRecord(c->ev[6], c->stream));
+    { const int rc = enqueue_chemistry(c, dt_s, true); if (rc != ARC_OK) return rc; }
     c->chem_once = true;
     // the rates stay valid as numbers, but they belong to the fields before this update
     if (!c->p.async) { CK(cudaStreamSynchronize(c->stream)); return check_pending(c); }
@@ -335,7 +403,9 @@ int arc_get_stats(arc_ctx *c, arc_stats *s)
     for (int v = 0; v < ARC_MAX_BINS; ++v) { s->emitted[v] = c->have_src ? c->emitted[v] : 0.0; s->absorbed[v] = ab[v]; s->escaped[v] = d.escaped[v]; }
     s->subcycles = d.subcycles; s->max_subcycles_cell = d.max_sub;
     s->trace_grid = c->trace_grid;
-    if (c->traced_once) {
+    s->segments_total = d.segments_total; s->subcycles_total = d.subcycles_total;
+    if (c->steps_timed) cudaEventElapsedTime(&s->steps_ms, c->ev_steps[0], c->ev_steps[1]);     // (per-kernel times: not inside a graph)
+    else if (c->traced_once) {
         cudaEventElapsedTime(&s->trace_ms, c->ev[0], c->ev[3]);
         cudaEventElapsedTime(&s->opacity_ms, c->ev[0], c->ev[1]);
         cudaEventElapsedTime(&s->trace_kernel_ms, c->ev[1], c->ev[2]);
@@ -345,7 +415,7 @@ int arc_get_stats(arc_ctx *c, arc_stats *s)
             s->trace_ms += s->finalize_ms;
         }
     }
-    if (c->chem_once) cudaEventElapsedTime(&s->chem_ms, c->ev[5], c->ev[6]);
+    if (c->chem_once && !c->steps_timed) cudaEventElapsedTime(&s->chem_ms, c->ev[5], c->ev[6]);
     s->kernel_launches = c->launches;
     cudaGetLastError();
     return check_pending(c);                    // (the statistics are filled in either way)

@@ -11,23 +11,15 @@ DECL_INST(f32_lo) DECL_INST(f32_hi) DECL_INST(f64_lo) DECL_INST(f64_hi)
 
 namespace {
 
-// scheduler reset before each trace: all root families are "in flight", queue empty, slot i expects ticket i
-// The error word is STICKY: an error a previous (asynchronous) trace left behind, which the host has not yet seen and
-// cleared (arc_check_device), stays - this trace then does not run and every consumer kernel keeps skipping.
-// `fault` = arc_params.debug_fault (test hook).
-__global__ void arc_sched_reset_kernel(SchedState *sc, DevStats *st, unsigned long long *qseq, unsigned long long seed_total, int fault)
+// Full reset of the donation queue: slot i expects ticket i, tickets start at 0.  Needed before the first trace and after
+// a trace that aborted; a trace that ends cleanly leaves the queue drained and consistent (every published ticket was
+// consumed, slot s then expects the next ticket that maps to it), so tickets simply keep counting from one trace to the
+// next and the 2 MB of slot words are not rewritten per trace.  The per-trace words are reset by arc_opacity_kernel.
+__global__ void arc_queue_reset_kernel(SchedState *sc, unsigned long long *qseq)
 {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < ARC_QUEUE_CAP) qseq[i] = i;
-    if (i == 0) {
-        sc->in_flight = (long long)seed_total; sc->seed_next = 0; sc->q_head = 0; sc->q_tail = 0;
-        if (sc->error == ARC_DEV_OK) sc->error = fault;
-        sc->hungry = 0; sc->q_high = 0; sc->log_n = 0; sc->q_count = 0;
-        st->segments = 0; st->rays = 0; st->digest = 0; st->deposit_records = 0;
-        for (int l = 0; l < ARC_MAX_LEVEL; ++l) { st->splits[l] = 0; st->rays_level[l] = 0; }
-        for (int e = 0; e < 3; ++e) st->ends[e] = 0;
-        for (int v = 0; v < ARC_MAX_BINS; ++v) st->escaped[v] = 0.0;
-    }
+    if (i == 0) { sc->q_head = 0; sc->q_tail = 0; sc->q_count = 0; sc->hungry = 0; }
 }
 
 __global__ void arc_pix2vec_kernel(const int32_t *level, const uint32_t *pix, int n, double *out)
@@ -145,9 +137,9 @@ cudaError_t arc_launch_pix2vec(const int32_t *d_level, const uint32_t *d_pix, in
     return cudaGetLastError();
 }
 
-cudaError_t arc_launch_sched_reset(arc_ctx *c, unsigned long long seed_total)
+cudaError_t arc_launch_queue_reset(arc_ctx *c)
 {
-    arc_sched_reset_kernel<<<ARC_QUEUE_CAP / 256, 256, 0, c->stream>>>(c->d_sched, c->d_stats, c->d_qseq, seed_total, c->p.debug_fault);
+    arc_queue_reset_kernel<<<ARC_QUEUE_CAP / 256, 256, 0, c->stream>>>(c->d_sched, c->d_qseq);
     ++c->launches;
     return cudaGetLastError();
 }

@@ -780,6 +780,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
     }
     if (lane == 0) {
         atomicAdd(&a.stats->segments, nseg);
+        atomicAdd(&a.stats->segments_total, nseg);
         atomicAdd(&a.stats->deposit_records, nred);
         if (FLAGS & FLAG_DIGEST) atomicAdd(&a.stats->digest, digest);
     }

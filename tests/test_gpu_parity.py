@@ -255,7 +255,7 @@ def test_kernel_launches_are_counted():
         n0 = cx.stats()["kernel_launches"]
         cx.trace(); cx.update_chemistry()
         n1 = cx.stats()["kernel_launches"]
-    assert n0 == 0 and n1 == 5          # reset, opacity + zero, tracer, finalize, chemistry
+    assert n0 == 0 and n1 == 5          # queue reset (first trace only), opacity + zero + reset, tracer, finalize, chemistry
 
 
 def test_ray_log_overflow_is_reported():
