@@ -42,6 +42,9 @@
 #endif
 #define FLAG_THIN 8         // template flag: track, per source, the radius up to which tau (bin 0) stays below thin_tau
 
+#ifndef ARC_GEOM_MIN_BLOCKS
+#define ARC_GEOM_MIN_BLOCKS 3      // ... of the variants with the geometric correction (measured: 2 blocks / 128 registers / no spills
+#endif                             // 56.4 G segments/s on config 4, 3 blocks / 80 registers / 200 B of spills 57.3: issue bound either way)
 #ifndef ARC_TRACE_MIN_BLOCKS
 #define ARC_TRACE_MIN_BLOCKS 3     // resident blocks per SM the register budget is held to (<= 85 registers)
 #endif
@@ -194,7 +197,7 @@ __device__ __forceinline__ float arc_ex2(float y)
 
 // ---------------------------------------------------------------------------------------------------
 template <int NB, typename KT, int FLAGS, int DEP>
-__global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_trace_kernel(const TraceArgs a)
+__global__ void __launch_bounds__(ARC_TRACE_THREADS, (FLAGS & FLAG_GEOM) ? ARC_GEOM_MIN_BLOCKS : ARC_TRACE_MIN_BLOCKS) arc_trace_kernel(const TraceArgs a)
 {
     typedef FamRec<NB> Rec;
     const int lane = threadIdx.x & 31;
@@ -414,6 +417,70 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
         // (the crossed axis), the advance costs one IEEE division, the next cell's opacities are requested before this
         // segment's attenuation arithmetic, and the state advance is unconditional (a lane that just ended is inactive).
         unsigned int nseg_b = 0, nred_b = 0;     // (nseg_b also is this ray's segment count: one ray per lane and batch)
+        // Geometric correction on the transposed route (GEOM_PIPE): the deposit runs ONE iteration late.  83 % of the shares
+        // that Eq. 3 hands to the adjacent cell go to the ray's own next or previous cell (measured on the oracle's ray
+        // logs, DESIGN.md 6.2 step 7): a share for the NEXT cell is carried in registers into the next segment's record, a
+        // share for the PREVIOUS cell is added to that cell's record while it still waits in the staging area, and only
+        // lateral shares need REDs of their own.  pcell = cell of the record waiting in my staging column.
+        constexpr bool GEOM_PIPE = ((FLAGS & FLAG_GEOM) != 0) && DEP == DEP_T;
+        [[maybe_unused]] double carry[NB];       // the share the last segment handed on (Eq. 3), until it has found its record
+        [[maybe_unused]] int pcell = -1 - lane;
+        [[maybe_unused]] bool have_carry = false; // ... it goes into this lane's next record
+        [[maybe_unused]] int entry = -1;          // code (2 axis + [direction > 0]) of the crossing that led into the current cell; -1: first segment
+        if constexpr (GEOM_PIPE) {
+#pragma unroll
+            for (int v = 0; v < NB; ++v) carry[v] = 0.0;
+        }
+        // DEP_T, stage 1: every lane writes its NB values into its column of the staging planes
+        auto stage_store = [&](double (&val)[NB]) {
+#pragma unroll
+            for (int v = 0; v < NB; ++v) asm volatile("st.shared.f64 [%0], %1;" ::"r"(dep_wr + (unsigned)(v * DEP_PLANE)), "d"(val[v]) : "memory");
+        };
+        // DEP_T, stage 2: in pass k = 0..3 the 4 lanes of quad q send the record of ray 4q + k, lane (q, b) issues bin b (and
+        // b + 4): the quad's REDs of one instruction fall in one 32-byte sector and leave the SM as one request - 2.5x the
+        // RED rate of one lane walking through the record.  `key` = the cell of the record in my column (negative: none).
+        auto stage_flush = [&](const int key) {
+            // the quad's 4 rays are siblings (or 4 neighbouring root pixels) less than a cell apart: rays of the quad that
+            // sit in the same cell are summed first (pure ALU work: the cells and values are in registers anyway), so a
+            // cell gets one record per quad and iteration
+            int cq[4];
+            double vq[(NB + 3) / 4][4];
+            // lane and bin from the (live) staging address instead of %tid (an S2R per iteration otherwise)
+            const unsigned ln = (dep_wr >> 3) & 31u, bq = ln & 3u;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                cq[k] = __shfl_sync(0xffffffffu, key, (ln & ~3u) + k);
+#pragma unroll
+                for (int b0 = 0; b0 < NB; b0 += 4) {
+                    vq[b0 / 4][k] = 0.0;
+                    if (b0 + 4 <= NB || b0 + bq < NB)
+                        asm volatile("ld.shared.f64 %0, [%1];" : "=d"(vq[b0 / 4][k]) : "r"(dep_rd + (unsigned)(b0 * DEP_PLANE + k * 8)) : "memory");
+                }
+            }
+            // sums first (all lanes, no branches), then four predicated REDs
+            bool first[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                first[k] = cq[k] >= 0;                           // not merged into an earlier ray of the quad
+#pragma unroll
+                for (int j = 0; j < k; ++j) first[k] = first[k] && (cq[j] != cq[k]);
+#pragma unroll
+                for (int j = k + 1; j < 4; ++j) {
+                    const bool same = cq[j] == cq[k];
+#pragma unroll
+                    for (int b0 = 0; b0 < NB; b0 += 4) vq[b0 / 4][k] += same ? vq[b0 / 4][j] : 0.0;
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                // record index in 32 bits where it fits (N <= 1024: cells < 2^30): one LEA + one wide multiply-add
+                double *Ac = (NBP <= 4) ? a.A + ((unsigned)cq[k] * (unsigned)NBP + bq) : a.A + (long long)cq[k] * NBP + bq;
+#pragma unroll
+                for (int b0 = 0; b0 < NB; b0 += 4)
+                    arc_red_add_if(Ac + b0, vq[b0 / 4][k], first[k] && (b0 + 4 <= NB || b0 + bq < NB));
+                if ((FLAGS & FLAG_DIGEST) && first[k] && bq == 0) ++nred_b;      // (statistic: digest builds only)
+            }
+        };
         KVec<KT, NB> kcur;
         kcur.load(kappa, cell);                 // (cell 0 for lanes without a ray: harmless)
         for (;;) {
@@ -422,6 +489,8 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
           int dcell = -1 - lane;                 // deposit key; lanes without a segment keep a unique negative one
           [[maybe_unused]] double avn[NB];       // FLAG_GEOM: what Eq. 3 hands to the adjacent cell ...
           [[maybe_unused]] int ncell = -1 - lane;  // ... and that cell (same convention as dcell)
+          [[maybe_unused]] int cls = 0;          // GEOM_PIPE: where that share goes: 0 nowhere, 1 my previous cell, 2 my next cell, 3 a lateral cell
+          [[maybe_unused]] int lat_code = 0;     // ... and the face it crosses (2 axis + upper)
           if (active) {
             // a6: first face crossed; ties go to x, then y (reading G9)
             int ax = 0; double tmin = tx;
@@ -516,11 +585,13 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                 // Geometric correction (readings G25-G29).  Which face is nearest decides where photons
                 // go, so that part is contract arithmetic (explicit round-to-nearest operations in the oracle's order):
                 // midpoint m_a = g_a + r_mid d_a, u_a = m_a - i_a, faces in the order x-, x+, y-, y+, z-, z+, first
-                // minimum wins; D_edge = max(min, 0); L_pix = r_mid (cpix 2^-l); f_c = 1/2 + D_edge / L_pix if
-                // 2 D_edge < L_pix, else 1.  The ray's own tau and P are not touched.
+                // minimum wins (taken per axis first - lower face unless the upper one is strictly nearer - then across the
+                // axes, x before y before z: the same face as the oracle's scan); D_edge = max(min, 0);
+                // L_pix = r_mid (cpix 2^-l); correction applies if 2 D_edge < L_pix.  The ray's own tau and P are not touched.
                 const double rmid = arc_mul(0.5, arc_add(r, r_out));
-                const double Lpix = arc_mul(rmid, scalbn(a.cpix, -level));
-                double D = INF; int nax = 0, nside = 0;
+                // cpix 2^-level: an exact power-of-two scaling, done on the exponent field (cpix ~ 1.02, level <= 14)
+                const double Lpix = arc_mul(rmid, __hiloint2double(__double2hiint(a.cpix) - (level << 20), __double2loint(a.cpix)));
+                double Dax[3]; int up[3];
 #pragma unroll
                 for (int ax3 = 0; ax3 < 3; ++ax3) {
                     double g3, d3;
@@ -528,25 +599,51 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                     asm volatile("ld.shared.f64 %0, [%1];" : "=d"(d3) : "r"(geo_ad + (unsigned)((3 + ax3) * ARC_TRACE_THREADS * 8)));
                     const double u = arc_sub(arc_add(g3, arc_mul(rmid, d3)), (double)((ijk >> (10 * ax3)) & 1023u));
                     const double hi = arc_sub(1.0, u);
-                    if (u < D) { D = u; nax = ax3; nside = -1; }
-                    if (hi < D) { D = hi; nax = ax3; nside = 1; }
+                    up[ax3] = hi < u;
+                    Dax[ax3] = up[ax3] ? hi : u;
                 }
-                if (D < 0.0) D = 0.0;
-                ncell = -1 - lane;
-                if (arc_mul(2.0, D) < Lpix) {
-                    double fc = arc_add(0.5, __ddiv_rn(D, Lpix));
-                    if (a.geom == ARC_GEOM_FC2) fc = arc_mul(fc, fc);
-                    const int jn = (int)((ijk >> (10 * nax)) & 1023u) + nside;
-                    const bool nb_in = (unsigned)jn < (unsigned)N;
-                    const int nstride = nax == 0 ? 1 : (nax == 1 ? N : a.NN);
-                    const bool move = (a.geom == ARC_GEOM_FC_SECONDARY) && nb_in;
-                    if (move) ncell = cell + nside * nstride;
+                double D = Dax[0]; int fcode = up[0];                       // face code = 2 axis + (upper face)
+                if (Dax[1] < D) { D = Dax[1]; fcode = 2 + up[1]; }
+                if (Dax[2] < D) { D = Dax[2]; fcode = 4 + up[2]; }
+                if (__double2hiint(D) < 0) D = 0.0;                         // (rounding can put the midpoint a hair outside)
+                bool corr = arc_mul(2.0, D) < Lpix;
+                // f_c = 1/2 + D_edge / L_pix (Eq. 2) only weighs the deposit - it decides nothing - so the quotient is taken in
+                // fp32 (1e-7 relative, far inside the tolerance; in + off = absorbed stays exact)
+                double fc = (double)(0.5f + fminf(__fdividef((float)D, (float)Lpix), 0.5f));      // (the quotient is < 1/2 where it is used)
+                if (a.geom == ARC_GEOM_FC2) fc = fc * fc;
+                const int nax = fcode >> 1;
+                const int jn = (int)((ijk >> (10 * nax)) & 1023u) + ((fcode & 1) ? 1 : -1);
+                const bool nb_in = (unsigned)jn < (unsigned)N;
+                // secondary correction with the neighbour outside the box: the cell keeps everything (G29)
+                if (a.geom == ARC_GEOM_FC_SECONDARY && !nb_in) corr = false;
+                if (!corr) fc = 1.0;                                        // (x 1.0 is exact: the deposit stays what it was)
+                const bool move = corr && (a.geom == ARC_GEOM_FC_SECONDARY);
+                if constexpr (GEOM_PIPE) {
+                    // where the share goes: my previous cell lies across the face I entered through, my next cell across the face
+                    // this segment ends on (if the ray goes on); anything else is a lateral cell
+                    if (move) cls = (entry >= 0 && fcode == (entry ^ 1)) ? 1 : ((go && !depleted && fcode == 2 * ax + pos) ? 2 : 3);
+                    lat_code = fcode;
+                    // this cell's record = its own (corrected) absorption + what the previous segment handed forward; the share
+                    // this segment hands on (Eq. 3) waits in `carry`
 #pragma unroll
                     for (int v = 0; v < NB; ++v) {
-                        const double in = fc * av[v], off = av[v] - in;
-                        avn[v] = off;                                         // (read only where ncell >= 0)
-                        // secondary correction with the neighbour outside the box: the cell keeps everything (G29)
-                        av[v] = (a.geom == ARC_GEOM_FC_SECONDARY && !nb_in) ? av[v] : in;
+                        double in = fc * av[v];
+                        const double off = av[v] - in;
+                        arc_add_if(in, carry[v], have_carry);
+                        av[v] = in;
+                        carry[v] = off;
+                    }
+                    have_carry = (cls == 2);
+                    entry = 2 * ax + pos;                                   // (the face the next segment enters through)
+                } else {
+                    ncell = -1 - lane;
+                    const int nstride = nax == 0 ? 1 : (nax == 1 ? N : a.NN);
+                    if (move) ncell = cell + ((fcode & 1) ? nstride : -nstride);
+#pragma unroll
+                    for (int v = 0; v < NB; ++v) {
+                        const double in = fc * av[v];
+                        avn[v] = av[v] - in;                                  // (read only where ncell >= 0)
+                        av[v] = in;
                     }
                 }
             }
@@ -580,7 +677,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
             ty = (ax == 1) ? t_new : ty;
             tz = (ax == 2) ? t_new : tz;
           }
-          // a7: deposit - the whole warp, converged (a lambda: the geometric correction runs the stage a second time)
+          // a7: deposit - the whole warp, converged
           auto deposit = [&](const int dcell, double (&av)[NB]) {
           if constexpr (DEP == DEP_AGG) {
               // segmented sum over the lanes that share a cell, by pointer jumping along each group's lane list:
@@ -605,52 +702,9 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
                   ++nred_b;
               }
           } else if constexpr (DEP == DEP_T) {
-              // every lane stages its NB absorbed rates; then, in pass k = 0..3, the 4 lanes of quad q send the record of
-              // ray 4q + k: lane (q, b) issues bin b (and b + 4): the quad's REDs of one instruction fall in one 32-byte
-              // sector and leave the SM as one request - 2.5x the RED rate of one lane walking through the record
-#pragma unroll
-              for (int v = 0; v < NB; ++v) asm volatile("st.shared.f64 [%0], %1;" ::"r"(dep_wr + (unsigned)(v * DEP_PLANE)), "d"(av[v]) : "memory");
+              stage_store(av);
               __syncwarp();
-              // the quad's 4 rays are siblings (or 4 neighbouring root pixels) less than a cell apart: rays of the quad that
-              // sit in the same cell are summed first (pure ALU work: the cells and values are in registers anyway), so a
-              // cell gets one record per quad and iteration
-              int cq[4];
-              double vq[(NB + 3) / 4][4];
-              // lane and bin from the (live) staging address instead of %tid (an S2R per iteration otherwise)
-              const unsigned ln = (dep_wr >> 3) & 31u, bq = ln & 3u;
-#pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                  cq[k] = __shfl_sync(0xffffffffu, dcell, (ln & ~3u) + k);
-#pragma unroll
-                  for (int b0 = 0; b0 < NB; b0 += 4) {
-                      vq[b0 / 4][k] = 0.0;
-                      if (b0 + 4 <= NB || b0 + bq < NB)
-                          asm volatile("ld.shared.f64 %0, [%1];" : "=d"(vq[b0 / 4][k]) : "r"(dep_rd + (unsigned)(b0 * DEP_PLANE + k * 8)) : "memory");
-                  }
-              }
-              // sums first (all lanes, no branches), then four predicated REDs
-              bool first[4];
-#pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                  first[k] = cq[k] >= 0;                           // not merged into an earlier ray of the quad
-#pragma unroll
-                  for (int j = 0; j < k; ++j) first[k] = first[k] && (cq[j] != cq[k]);
-#pragma unroll
-                  for (int j = k + 1; j < 4; ++j) {
-                      const bool same = cq[j] == cq[k];
-#pragma unroll
-                      for (int b0 = 0; b0 < NB; b0 += 4) vq[b0 / 4][k] += same ? vq[b0 / 4][j] : 0.0;
-                  }
-              }
-#pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                  // record index in 32 bits where it fits (N <= 1024: cells < 2^30): one LEA + one wide multiply-add
-                  double *Ac = (NBP <= 4) ? a.A + ((unsigned)cq[k] * (unsigned)NBP + bq) : a.A + (long long)cq[k] * NBP + bq;
-#pragma unroll
-                  for (int b0 = 0; b0 < NB; b0 += 4)
-                      arc_red_add_if(Ac + b0, vq[b0 / 4][k], first[k] && (b0 + 4 <= NB || b0 + bq < NB));
-                  if ((FLAGS & FLAG_DIGEST) && first[k] && bq == 0) ++nred_b;      // (statistic: digest builds only)
-              }
+              stage_flush(dcell);
               __syncwarp();                       // rows are rewritten in the next iteration
           } else {
               if (dcell >= 0) {
@@ -661,10 +715,42 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, ARC_TRACE_MIN_BLOCKS) arc_t
               }
           }
           };
-          deposit(dcell, av);
-          if constexpr ((FLAGS & FLAG_GEOM) != 0) {
-              if (__any_sync(0xffffffffu, ncell >= 0)) deposit(ncell, avn);        // Eq. 3: the adjacent cells' share
+          if constexpr (GEOM_PIPE) {
+              // the record in my staging column is that of my PREVIOUS segment (cell pcell): a share for that cell joins it there
+              // (own column: no other lane writes it, and the quad read it before the last __syncwarp)
+              if (cls == 1) {
+#pragma unroll
+                  for (int v = 0; v < NB; ++v) {
+                      double x;
+                      asm volatile("ld.shared.f64 %0, [%1];" : "=d"(x) : "r"(dep_wr + (unsigned)(v * DEP_PLANE)) : "memory");
+                      x += carry[v];
+                      asm volatile("st.shared.f64 [%0], %1;" ::"r"(dep_wr + (unsigned)(v * DEP_PLANE)), "d"(x) : "memory");
+                  }
+              }
+              if (cls == 3) {                     // a lateral cell: REDs of its own (one lane, NB doubles of one record)
+                  const int lax = lat_code >> 1, lstride = lax == 0 ? 1 : (lax == 1 ? N : a.NN);
+                  double *An = a.A + (long long)(dcell + ((lat_code & 1) ? lstride : -lstride)) * NBP;
+#pragma unroll
+                  for (int v = 0; v < NB; ++v) arc_red_add(An + v, carry[v]);
+                  ++nred_b;
+              }
+              __syncwarp();
+              stage_flush(pcell);                 // the records of the previous iteration, complete now
+              __syncwarp();
+              stage_store(av);                    // this iteration's records wait for the next one
+              pcell = dcell;
+          } else {
+              deposit(dcell, av);
+              if constexpr ((FLAGS & FLAG_GEOM) != 0) {
+                  if (__any_sync(0xffffffffu, ncell >= 0)) deposit(ncell, avn);        // Eq. 3: the adjacent cells' share
+              }
           }
+        }
+        if constexpr (GEOM_PIPE) {
+            // the records of the last iteration are still waiting
+            __syncwarp();
+            stage_flush(pcell);
+            __syncwarp();
         }
         nseg += nseg_b; nred += nred_b;
         __syncwarp();
