@@ -25,7 +25,8 @@ ARC_GEOM_NONE, ARC_GEOM_FC, ARC_GEOM_FC_SECONDARY, ARC_GEOM_FC2 = 0, 1, 2, 3
 ARC_MAX_BINS, ARC_MAX_LEVEL = 8, 16
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libarc_b200.so")
+# ARC_B200_LIB: another build of the same library, e.g. libarc_b200_checked.so (device-side bounds checks)
+LIB_PATH = os.environ.get("ARC_B200_LIB") or os.path.join(_HERE, "libarc_b200.so")
 
 EXPORTS = ["arc_create_grid", "arc_destroy", "arc_default_params", "arc_set_params", "arc_set_stream",
            "arc_set_fields", "arc_get_fields", "arc_set_spectrum", "arc_set_sources", "arc_set_emission_mask", "arc_get_thin_radii", "arc_set_thin_radii", "arc_trace",

@@ -15,6 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libarc_b200.so")
+LIB_CHECKED = os.path.join(HERE, "libarc_b200_checked.so")       # -DARC_CHECKED=1: device-side bounds checks (csrc/arc_internal.cuh)
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]                 # cudart: static (nvcc default), self-contained
@@ -28,10 +29,11 @@ def _deps():
     return sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + [os.path.join(HERE, "..", "include", "arc.h")]
 
 
-def needs_build() -> bool:
-    if not os.path.exists(LIB):
+def needs_build(checked: bool = False) -> bool:
+    lib = LIB_CHECKED if checked else LIB
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     return any(os.path.getmtime(p) > t for p in _deps())
 
 
@@ -43,20 +45,22 @@ def nvcc_path() -> str:
 
 
 def _compile_one(args):
-    src, obj, verbose = args
-    cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
+    src, obj, verbose, checked = args
+    cmd = [nvcc_path()] + NVCC_FLAGS + (["-DARC_CHECKED=1"] if checked else []) + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
     r = subprocess.run(cmd, capture_output=True, text=True)
     return src, r.returncode, " ".join(cmd) + "\n" + r.stdout + r.stderr
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile every csrc/*.cu to an object (in parallel: the tracer's instantiation units dominate) and link."""
-    if not force and not needs_build():
+def build(force: bool = False, verbose: bool = False, checked: bool = False) -> str:
+    """Compile every csrc/*.cu to an object (in parallel: the tracer's instantiation units dominate) and link.
+    checked = True: the same sources with -DARC_CHECKED=1 into libarc_b200_checked.so."""
+    LIB = LIB_CHECKED if checked else globals()["LIB"]
+    if not force and not needs_build(checked):
         return LIB
     from concurrent.futures import ThreadPoolExecutor
-    objdir = os.path.join(HERE, "build")
+    objdir = os.path.join(HERE, "build", "checked" if checked else "")
     os.makedirs(objdir, exist_ok=True)
-    jobs = [(s, os.path.join(objdir, os.path.basename(s)[:-3] + ".o"), verbose) for s in sources()]
+    jobs = [(s, os.path.join(objdir, os.path.basename(s)[:-3] + ".o"), verbose, checked) for s in sources()]
     with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
         results = list(ex.map(_compile_one, jobs))
     for src, rc, log in results:
@@ -72,4 +76,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, checked="--checked" in sys.argv))

@@ -28,7 +28,11 @@ static size_t esize(const arc_ctx *c) { return c->dtype == ARC_F32 ? 4 : 8; }
 
 extern "C" {
 
-const char *arc_version(void) { return "arc-b200 0.1 (sm_100a)"; }
+#ifdef ARC_CHECKED
+const char *arc_version(void) { return "arc-b200 0.2 (sm_100a, checked build)"; }
+#else
+const char *arc_version(void) { return "arc-b200 0.2 (sm_100a)"; }
+#endif
 
 const char *arc_last_error(const arc_ctx *c) { return c ? c->err.c_str() : g_create_err.c_str(); }
 

@@ -15,7 +15,18 @@
 #define ARC_BATCH_FAM 8              // families (x4 children = 32 rays) per warp batch
 
 // device-side error codes written to SchedState::error
-enum { ARC_DEV_OK = 0, ARC_DEV_STACK_OVERFLOW = 1, ARC_DEV_LOG_OVERFLOW = 2, ARC_DEV_WATCHDOG = 3, ARC_DEV_RAY_RUNAWAY = 4 };
+enum { ARC_DEV_OK = 0, ARC_DEV_STACK_OVERFLOW = 1, ARC_DEV_LOG_OVERFLOW = 2, ARC_DEV_WATCHDOG = 3, ARC_DEV_RAY_RUNAWAY = 4,
+       ARC_DEV_CHECK_FAILED = 5 };   // (5: a bounds check of the checked build, -DARC_CHECKED=1: libarc_b200_checked.so)
+
+// The checked build (paper_1807_07094_b200/build.py --checked; tests/test_gpu_checked_build.py runs parity workloads
+// through it) verifies, on the device, every index the tracer forms before it is used: cells, sources, levels, ring and
+// queue slots, staging addresses, log entries.  compute-sanitizer is not available on the pool this was developed on
+// (profiles/r02_sanitizers.md), so the kernel checks itself.  In the normal build ARC_CHECK compiles to nothing.
+#ifdef ARC_CHECKED
+#define ARC_CHECK(sc_, cond) do { if (!(cond)) atomicCAS(&(sc_)->error, 0, ARC_DEV_CHECK_FAILED); } while (0)
+#else
+#define ARC_CHECK(sc_, cond) do { } while (0)
+#endif
 
 // A "family" = the 4 children 4*fam+j (j = 0..3) of one split (or 4 consecutive root pixels), all at
 // `level`, starting at the parent's split radius with the parent's optical depths.  P is the

@@ -36,6 +36,7 @@ int arc_check_device(arc_ctx *c)
         case ARC_DEV_LOG_OVERFLOW: return fail(c, ARC_EOVERFLOW, "arc_trace_debug: ray log too small");
         case ARC_DEV_WATCHDOG: return fail(c, ARC_ECUDA, "arc_trace: scheduler watchdog fired (no progress for 20 s); rates are invalid");
         case ARC_DEV_RAY_RUNAWAY: return fail(c, ARC_ECUDA, "arc_trace: a ray exceeded 3N+8 segments; rates are invalid");
+        case ARC_DEV_CHECK_FAILED: return fail(c, ARC_ECUDA, "arc_trace: a bounds check of the checked build failed; rates are invalid");
         default: return fail(c, ARC_ECUDA, "arc_trace: kernel ended with work still in flight; rates are invalid");
     }
 }

@@ -287,6 +287,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, (FLAGS & FLAG_GEOM) ? ARC_G
                     if (lane < n) {
                         const unsigned long long tk = ticket + lane;
                         const unsigned slot = (unsigned)(tk % ARC_QUEUE_CAP);
+                        ARC_CHECK(sc, top + lane - bot < ARC_STACK_CAP);
                         while (ld_volatile_u64(&a.qseq[slot]) != tk + 1) __nanosleep(32);
                         __threadfence();
                         const int4 *src = reinterpret_cast<const int4 *>(&queue[slot]);
@@ -322,6 +323,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, (FLAGS & FLAG_GEOM) ? ARC_G
                             r.src = (uint32_t)lo; r.fam = (uint32_t)(s - __ldg(a.seed_prefix + lo));
                             r.level = (uint32_t)__ldg(a.src_level + lo);
                         }
+                        ARC_CHECK(sc, r.src < (uint32_t)a.nsrc && r.level <= (uint32_t)a.Lmax && r.fam < (3u << (2 * r.level)) && top + lane - bot < ARC_STACK_CAP);
                         r.pad = 1;                                        // root family: starts at Rstart[src] (0 without a thin region)
                         const double npix0 = (double)(12ull << (2 * r.level));
 #pragma unroll
@@ -377,6 +379,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, (FLAGS & FLAG_GEOM) ? ARC_G
         if (active) {
             const Rec *rp = &STK(top + myfam);
             src = rp->src; level = (int)rp->level; pix = 4u * rp->fam + (uint32_t)(lane & 3);
+            ARC_CHECK(sc, src < (uint32_t)a.nsrc && level >= 0 && level < ARC_MAX_LEVEL && level <= a.Lmax && (unsigned long long)pix < (12ull << (2 * level)));
 #pragma unroll
             for (int v = 0; v < NB; ++v) { tau[v] = rp->tau[v]; P[v] = rp->P[v]; }
             double dirx, diry, dirz;
@@ -440,6 +443,9 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, (FLAGS & FLAG_GEOM) ? ARC_G
         // b + 4): the quad's REDs of one instruction fall in one 32-byte sector and leave the SM as one request - 2.5x the
         // RED rate of one lane walking through the record.  `key` = the cell of the record in my column (negative: none).
         auto stage_flush = [&](const int key) {
+            ARC_CHECK(sc, key < a.NN * N);
+            if constexpr (DEP == DEP_T) ARC_CHECK(sc, dep_wr + (unsigned)((NB - 1) * DEP_PLANE) + 8u <= (unsigned)__cvta_generic_to_shared(s_dep) + (unsigned)sizeof(s_dep)
+                                                   && dep_rd + (unsigned)(((NB - 1) / 4 * 4) * DEP_PLANE) + 32u <= (unsigned)__cvta_generic_to_shared(s_dep) + (unsigned)sizeof(s_dep) + 3u * DEP_PLANE);
             // the quad's 4 rays are siblings (or 4 neighbouring root pixels) less than a cell apart: rays of the quad that
             // sit in the same cell are summed first (pure ALU work: the cells and values are in registers anyway), so a
             // cell gets one record per quad and iteration
@@ -482,6 +488,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, (FLAGS & FLAG_GEOM) ? ARC_G
             }
         };
         KVec<KT, NB> kcur;
+        ARC_CHECK(sc, (unsigned)cell < (unsigned)(a.NN * N));
         kcur.load(kappa, cell);                 // (cell 0 for lanes without a ray: harmless)
         for (;;) {
           if (!__any_sync(0xffffffffu, active)) break;
@@ -518,6 +525,8 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, (FLAGS & FLAG_GEOM) ? ARC_G
             if (ax == 0) stride = 1;
             const int cell_next = cell + st * stride;
             const bool go = !(split || out);
+            ARC_CHECK(sc, (unsigned)cell < (unsigned)(a.NN * N) && (!go || (unsigned)cell_next < (unsigned)(a.NN * N)) && ax >= 0 && ax <= 2);
+            ARC_CHECK(sc, cell == (int)(((ijk >> 20) & 1023u) * (unsigned)N + ((ijk >> 10) & 1023u)) * N + (int)(ijk & 1023u));
             const double t_new = arc_div_by_recip(arc_sub((double)(inext + pos), g_ax), d_ax, y_ax);   // == IEEE division (C3)
             // a7: optical depth (fp64, decides: contract C4) and the deposit of Eq. 1
             bool depleted = true;
@@ -696,6 +705,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, (FLAGS & FLAG_GEOM) ? ARC_G
               }
               const bool head = (lane == leader);
               if (head && dcell >= 0) {
+                  ARC_CHECK(sc, dcell < a.NN * N);
                   double *Ac = a.A + (long long)dcell * NBP;
 #pragma unroll
                   for (int v = 0; v < NB; ++v) arc_red_add(Ac + v, av[v]);
@@ -708,6 +718,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, (FLAGS & FLAG_GEOM) ? ARC_G
               __syncwarp();                       // rows are rewritten in the next iteration
           } else {
               if (dcell >= 0) {
+                  ARC_CHECK(sc, dcell < a.NN * N);
                   double *Ac = a.A + (long long)dcell * NBP;
 #pragma unroll
                   for (int v = 0; v < NB; ++v) arc_red_add(Ac + v, av[v]);   // a7: REDG.E.ADD.F64 ("atomically")
@@ -729,6 +740,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, (FLAGS & FLAG_GEOM) ? ARC_G
               }
               if (cls == 3) {                     // a lateral cell: REDs of its own (one lane, NB doubles of one record)
                   const int lax = lat_code >> 1, lstride = lax == 0 ? 1 : (lax == 1 ? N : a.NN);
+                  ARC_CHECK(sc, (unsigned)(dcell + ((lat_code & 1) ? lstride : -lstride)) < (unsigned)(a.NN * N));
                   double *An = a.A + (long long)(dcell + ((lat_code & 1) ? lstride : -lstride)) * NBP;
 #pragma unroll
                   for (int v = 0; v < NB; ++v) arc_red_add(An + v, carry[v]);
@@ -799,6 +811,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, (FLAGS & FLAG_GEOM) ? ARC_G
         } else {
             if (do_split) {
                 const int rank = __popc(ballot & ((1u << lane) - 1u));
+                ARC_CHECK(sc, level + 1 <= a.Lmax && top + rank - bot < ARC_STACK_CAP);
                 Rec rec;
                 rec.src = src; rec.fam = pix; rec.level = (uint32_t)(level + 1); rec.pad = 0;
 #pragma unroll
@@ -840,6 +853,7 @@ __global__ void __launch_bounds__(ARC_TRACE_THREADS, (FLAGS & FLAG_GEOM) ? ARC_G
                 if (lane < nd) {
                     const unsigned long long tk = ticket + lane;
                     const unsigned slot = (unsigned)(tk % ARC_QUEUE_CAP);
+                    ARC_CHECK(sc, bot + lane < top);
                     while (ld_volatile_u64(&a.qseq[slot]) != tk) __nanosleep(32);    // previous lap's reader finished
                     const int4 *s4 = reinterpret_cast<const int4 *>(&STK(bot + lane));
                     int4 *d4 = reinterpret_cast<int4 *>(&queue[slot]);
