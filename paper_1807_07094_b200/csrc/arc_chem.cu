@@ -322,7 +322,12 @@ cudaError_t launch_chem(arc_ctx *c, double dt)
     const ChemK q = chem_consts(c->p.caseB != 0, c->p.coll_ion != 0);
     const long long nb = (c->ncell + 127) / 128;
     if (c->p.isothermal) {
-        const long long cap = (long long)c->n_sm * 32;
+        // exactly the co-resident blocks, grid-stride: every block evaluates the rate table once (a chain of a thousand
+        // dependent fp64 instructions), so blocks beyond one wave would only repeat that latency
+        int per_sm = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, arc_chem_iso_kernel<FT>, 128, 0);
+        if (e != cudaSuccess) return e;
+        const long long cap = (long long)c->n_sm * (per_sm > 0 ? per_sm : 1);
         arc_chem_iso_kernel<FT><<<(int)(nb < cap ? nb : cap), 128, 0, c->stream>>>(c->ncell, dt, c->p.Yp, c->p.eps_sub, c->p.x_floor, c->p.max_subcycles,
                                                                                  q, f[0], f[1], f[2], f[3], f[4], c->d_rates, c->d_stats, c->d_sched);
     } else {
