@@ -13,7 +13,7 @@ import pytest
 
 from oracle import oracle as orc
 from paper_1807_07094_b200 import arc, workloads as wl
-from gpu_common import RTOL, assert_close, compare_trace_stats
+from gpu_common import RTOL, assert_close, compare_trace_stats, oracle_trace_parallel
 
 pytestmark = pytest.mark.gpu
 
@@ -91,8 +91,7 @@ def _stats_ints(st):
 def _sampled_source_parity(w, sample, rtol, fields=None):
     """the oracle and the CUDA path each trace the sources `sample` alone on the same fields"""
     fields = fields if fields is not None else w.fields()
-    kappa = orc.opacity(w, fields)
-    Ao, so, _ = orc.trace(w, kappa=kappa, sources=sample)
+    Ao, so = oracle_trace_parallel(w, fields=fields, sources=sample, threads=8)      # (the unchanged oracle, on disjoint shares of the root rays)
     with arc.Context(w, fields=fields, digest=1) as cx:
         cx.set_sources(sample)
         cx.trace()
