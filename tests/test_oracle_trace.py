@@ -194,6 +194,42 @@ def test_finalize_partition_of_unity_and_single_species():
     assert np.all(G1[1:] == 0)
 
 
+def test_finalize_of_a_hand_worked_three_species_cell():
+    """orc_finalize with all three absorbers and three bins, numbers worked by hand (Eq. 1 with n_abs = n_SI, PAPER.md:83;
+    heating h(nu - nu_S) s_nu n_SI; the species' share of a bin is its share of the opacity, reading G8).
+    Y_p = 0.2: n_He = n_H/16.  Cell: n_H = 1.6e-2, x = (0.5, 0.25, 0.5) -> n_HI = 8e-3, n_HeI = 2.5e-4, n_HeII = 5e-4;
+    kappa = (4.8e-20, 1.7e-20, 9e-21) cm^-1 (tests/test_oracle_chem_pins.py works those out)."""
+    w = wl.tiny(N=2, nb=3, dtype="f64")
+    w.E_eV = np.array([20.0, 40.0, 80.0])
+    w.sig_HI = np.array([6e-18, 2e-18, 1e-18]); w.sig_HeI = np.array([0.0, 4e-18, 2e-18]); w.sig_HeII = np.array([0.0, 0.0, 1e-18])
+    f = (np.full(8, 1.6e-2), np.full(8, 0.5), np.full(8, 0.25), np.full(8, 0.5), np.full(8, 1e4))
+    A = np.zeros((8, 3)); A[0] = (3e40, 2e40, 1e40)
+    G, H, Ht = orc.finalize(w, A, f, Yp=0.2)
+    V = (w.box_cm / 2) ** 3
+    eV = 1.602176634e-12
+    per_bin_HI = np.array([3e40 * 6e-18 / 4.8e-20, 2e40 * 2e-18 / 1.7e-20, 1e40 * 1e-18 / 9e-21])       # 3.75e42, 2.3529e42, 1.1111e42
+    per_bin_HeI = np.array([0.0, 2e40 * 4e-18 / 1.7e-20, 1e40 * 2e-18 / 9e-21])
+    per_bin_HeII = np.array([0.0, 0.0, 1e40 * 1e-18 / 9e-21])
+    assert abs(G[0, 0] * V / 7.214052e42 - 1) < 1e-6 and abs(G[0, 0] * V / per_bin_HI.sum() - 1) < 1e-13
+    assert abs(G[1, 0] * V / per_bin_HeI.sum() - 1) < 1e-13 and abs(G[2, 0] * V / per_bin_HeII.sum() - 1) < 1e-13
+    # every absorbed photon ionises exactly one atom: sum_S Gamma_S n_S V = sum_nu A_nu = 6e40
+    assert abs((G[0, 0] * 8e-3 + G[1, 0] * 2.5e-4 + G[2, 0] * 5e-4) * V / 6e40 - 1) < 1e-13
+    # heating per absorber: photon energy above each species' OWN threshold (13.598, 24.587, 54.418 eV)
+    want_H = [(per_bin_HI * (w.E_eV - 13.598)).sum(), (per_bin_HeI * (w.E_eV - 24.587)).sum(), (per_bin_HeII * (w.E_eV - 54.418)).sum()]
+    assert abs(want_H[0] / 1.599099e44 - 1) < 1e-6 and abs(want_H[1] / 1.956718e44 - 1) < 1e-6 and abs(want_H[2] / 2.842444e43 - 1) < 1e-6
+    for S in range(3):
+        assert abs(H[S, 0] * V / (want_H[S] * eV) - 1) < 1e-13, S
+    assert abs(Ht[0] / (H[0, 0] * 8e-3 + H[1, 0] * 2.5e-4 + H[2, 0] * 5e-4) - 1) < 1e-13
+    assert np.all(G[:, 1:] == 0) and np.all(Ht[1:] == 0)
+    # a bin below a species' threshold ionises nothing of it by construction (sigma = 0); if a caller gives it a
+    # cross-section anyway, the photons are counted but heat nothing (no negative heating)
+    w.sig_HeI = np.array([1e-18, 4e-18, 2e-18])
+    G2, H2, _ = orc.finalize(w, A, f, Yp=0.2)
+    k0 = 6e-18 * 8e-3 + 1e-18 * 2.5e-4
+    assert abs(G2[1, 0] * V / (3e40 * 1e-18 / k0 + per_bin_HeI[1:].sum()) - 1) < 1e-13
+    assert abs(H2[1, 0] / H[1, 0] - 1) < 1e-13
+
+
 def test_flux_unit_arithmetic_from_the_paper():
     # PAPER.md:245 and :298 - the paper's own worked numbers pin the unit constants of the input module
     vals = dict(l.split()[:2] for l in open(__file__.rsplit("/", 1)[0] + "/golden/paper_values.txt")
