@@ -15,7 +15,7 @@ time against the measured HBM copy bandwidth - the figure BASELINE.json asks for
 in-quad merge of deposits keep most of those bytes off DRAM, so the line also carries what binds the kernel:
 `issue` (warp instructions per second against 4 schedulers x SMs x SM clock) and `roofline.dram_frac` (ncu DRAM bytes
 over the same time) - both from the committed ncu capture profiles/ncu_traffic.json, used only if that capture is of
-this workload, these flags and this build of csrc/ (else null).
+this workload, these flags and this build of the tracer's sources (else null).
 
 With --gpus N > 1 and no torchrun environment the script starts its own N ranks (torch.distributed.run, 127.0.0.1).
 """
@@ -77,19 +77,22 @@ def hbm_peak():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+TRACER_SOURCES = ("arc_trace_kernel.cuh", "arc_healpix.cuh", "arc_divide.cuh", "arc_internal.cuh", "arc_trace.cu",
+                  "arc_trace_inst_f32_lo.cu", "arc_trace_inst_f32_hi.cu", "arc_trace_inst_f64_lo.cu", "arc_trace_inst_f64_hi.cu")
+
+
 def csrc_sha16() -> str:
-    """identifies the build of the CUDA sources an ncu capture belongs to"""
-    import glob
+    """identifies the build of the TRACER's sources an ncu capture of the tracer belongs to"""
     h = hashlib.sha256()
-    for f in sorted(glob.glob(os.path.join(ROOT, "paper_1807_07094_b200", "csrc", "*.cu*"))):
-        h.update(os.path.basename(f).encode()); h.update(open(f, "rb").read())
+    for f in TRACER_SOURCES:
+        h.update(f.encode()); h.update(open(os.path.join(ROOT, "paper_1807_07094_b200", "csrc", f), "rb").read())
     return h.hexdigest()[:16]
 
 
 def ncu_capture(workload: str, segments_per_launch: float, flags: dict):
     """-> (capture dict or None, reason).  profiles/ncu_traffic.json holds, per workload, what one committed
     `ncu --set full` capture of the tracer measured (DRAM bytes, warp instructions per launch).  It is used only when it
-    is a capture of THIS workload (same segments per launch), THESE flags and THIS build of csrc/."""
+    is a capture of THIS workload (same segments per launch), THESE flags and THIS build of the tracer's sources."""
     try:
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
             cap = json.load(f).get(workload)
@@ -102,8 +105,8 @@ def ncu_capture(workload: str, segments_per_launch: float, flags: dict):
     if int(cap.get("segments_per_launch", -1)) != int(round(segments_per_launch)):
         return None, "the committed capture traced a different number of segments"
     if cap.get("csrc_sha16") != csrc_sha16():
-        return None, f"the committed capture ({cap.get('capture')}) is of another build of csrc/"
-    return cap, f"{cap.get('capture')} (ncu --set full, one launch, same workload / flags / csrc build {cap.get('csrc_sha16')})"
+        return None, f"the committed capture ({cap.get('capture')}) is of another build of the tracer's sources"
+    return cap, f"{cap.get('capture')} (ncu --set full, one launch, same workload / flags / tracer sources {cap.get('csrc_sha16')})"
 
 
 def algorithmic_bytes_per_segment(w) -> int:

@@ -38,10 +38,36 @@ struct ChemK {
     int coll, p_rec_is_15;
 };
 
+// e^x with 1.5e-7 relative error for the fp32-field mode (tolerance 1e-3): x log2(e) = k + f with k = round
+// and |f| <= 1/2, 2^f on the SFU (ex2.approx.f32: 2 ulp of fp32), the float widened and scaled by 2^k with integer
+// operations on its bit pattern (no conversion instruction: those share the SFU's pipe).  Nine instructions against the
+// ~28 of the fp64 exp.  Below e^-700 the result is 0 (the fits multiply it by numbers of order 1e-10 .. 1e+2).
+__device__ __forceinline__ double exp_sfu(double x)
+{
+    const double MAGIC = 6755399441055744.0;                           // 1.5 * 2^52: round to nearest integer
+    const double t = x * 1.4426950408889634074;
+    const double kt = t + MAGIC;
+    const int k = __double2loint(kt);
+    const float f = (float)(t - (kt - MAGIC));
+    float p;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(p) : "f"(f));            // in [0.707, 1.415]: a normal float
+    const unsigned b = __float_as_uint(p);
+    const double r = __hiloint2double((int)(b >> 3) + ((896 + k) << 20), (int)(b << 29));      // (double)p * 2^k
+    return x < -700.0 ? 0.0 : r;
+}
+
+template <bool FAST> struct RtMath;
+template <> struct RtMath<false> { static __device__ __forceinline__ double ex(double x) { return exp(x); } };
+template <> struct RtMath<true> { static __device__ __forceinline__ double ex(double x) { return exp_sfu(x); } };
+
+// FAST (fp32-field runs): the exponentials of the fits from exp_sfu; the logarithms stay fp64 (they sit in exponents: an
+// absolute error of 2e-7 there would be a relative error of up to 1e-6 in the rate)
+template <bool FAST = false>
 __device__ __forceinline__ void rate_table(double T, const ChemK &q, Coef &k)
 {
     const double KB = 1.380649e-16;
     const double TR_H = 157807.0, TR_HE1 = 285335.0, TR_HE2 = 631515.0;   // ionisation thresholds in K
+    auto exp = [](double x) { return RtMath<FAST>::ex(x); };             // (shadows ::exp inside this function)
     const double L = log(T), iT = 1.0 / T;
     // recombination and its cooling: A0 lambda^p / (1 + (lambda/l0)^q)^s
     const double ep = exp(-q.p_rec * L), eq = exp(-q.q_rec * L);
@@ -103,7 +129,7 @@ struct Cell {
 };
 
 // one sub-cycle of PAPER.md:136-154 (readings G12, G15-G17, G23, G24); k = rate table at c.T (ISO: evaluated by the caller)
-template <bool ISO>
+template <bool ISO, bool FAST = false>
 __device__ __forceinline__ void chem_subcycle(Cell &c, Coef &k, const ChemK &q, double dt, double eps, double x_floor, int max_sub)
 {
     const double KB = 1.380649e-16;
@@ -113,7 +139,7 @@ __device__ __forceinline__ void chem_subcycle(Cell &c, Coef &k, const ChemK &q, 
     const double xHII = 1.0 - x0;
     double xHeIII = 1.0 - x1 - x2; if (xHeIII < 0.0) xHeIII = 0.0;
     const double ne = nH * xHII + nHe * (x2 + 2.0 * xHeIII);
-    if (!ISO) rate_table(c.T, q, k);
+    if (!ISO) rate_table<FAST>(c.T, q, k);
     // Eq. 4 written as Eq. 5 (dn/dt = D - C n), in fractions
     const double C0 = c.G0 + k.cHI * ne,              D0 = k.aHII * ne * xHII;
     const double C1 = c.G1 + k.cHeI * ne,             D1 = k.aHeII * ne * x2;
@@ -242,7 +268,7 @@ __global__ void __launch_bounds__(128, 5) arc_chem_kernel(long long ncell, doubl
         }
         if (__all_sync(0xffffffffu, mine < 0)) break;
         if (mine >= 0) {
-            if (c.t < dt && c.n < max_sub) chem_subcycle<false>(c, k, q, dt, eps, x_floor, max_sub);
+            if (c.t < dt && c.n < max_sub) chem_subcycle<false, sizeof(FT) == 4>(c, k, q, dt, eps, x_floor, max_sub);
             if (!(c.t < dt && c.n < max_sub)) {
                 xHIf[mine] = (FT)c.x0; xHeIf[mine] = (FT)c.x1; xHeIIf[mine] = (FT)c.x2; Tf[mine] = (FT)c.T;
                 my_sub += (unsigned long long)c.n;

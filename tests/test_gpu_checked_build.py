@@ -22,7 +22,7 @@ def test_parity_suite_through_the_checked_build():
                            capture_output=True, text=True, cwd=ROOT, env=env)
     assert "checked build" in probe.stdout, probe.stdout + probe.stderr
     sel = ("tiny_random or four_bin_f32 or small_persistent or many_sources or faces_edges or parameter_variants or "
-           "repeatable or tiny_workloads or mask or thin or config1_per_ray")
+           "repeatable or tiny_workloads or masked_sources or config1_per_ray or two_traces_radii or injected_radii or config1_steps")
     r = subprocess.run([sys.executable, "-m", "pytest", "-q", "-x", "-m", "gpu", "-p", "no:cacheprovider", "tests/test_gpu_parity.py",
                         "tests/test_gpu_geom.py", "tests/test_gpu_mask.py", "tests/test_gpu_thin.py", "-k", sel],
                        capture_output=True, text=True, cwd=ROOT, env=env, timeout=1800)
