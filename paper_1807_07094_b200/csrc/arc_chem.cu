@@ -38,36 +38,80 @@ struct ChemK {
     int coll, p_rec_is_15;
 };
 
-// e^x with 1.5e-7 relative error for the fp32-field mode (tolerance 1e-3): x log2(e) = k + f with k = round
-// and |f| <= 1/2, 2^f on the SFU (ex2.approx.f32: 2 ulp of fp32), the float widened and scaled by 2^k with integer
-// operations on its bit pattern (no conversion instruction: those share the SFU's pipe).  Nine instructions against the
-// ~28 of the fp64 exp.  Below e^-700 the result is 0 (the fits multiply it by numbers of order 1e-10 .. 1e+2).
-__device__ __forceinline__ double exp_sfu(double x)
+// e^x for the rate table, 3e-13 relative: x = k ln2 + r with |r| <= ln2 / 2 (two-part ln2), the Taylor polynomial of degree 10
+// in Horner form, scaled by 2^k on the exponent field.  No special cases (the fits never pass it a NaN or more than +60;
+// below e^-700 the result is 0: the fits multiply it by numbers of order 1e-10 .. 1e+2) - 19 instructions against the ~30 of
+// the library's exp, which the table calls 18-26 times per sub-cycle.
+__device__ __forceinline__ double exp_table(double x)
 {
     const double MAGIC = 6755399441055744.0;                           // 1.5 * 2^52: round to nearest integer
-    const double t = x * 1.4426950408889634074;
-    const double kt = t + MAGIC;
+    const double kt = fma(x, 1.4426950408889634074, MAGIC);
     const int k = __double2loint(kt);
-    const float f = (float)(t - (kt - MAGIC));
-    float p;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(p) : "f"(f));            // in [0.707, 1.415]: a normal float
-    const unsigned b = __float_as_uint(p);
-    const double r = __hiloint2double((int)(b >> 3) + ((896 + k) << 20), (int)(b << 29));      // (double)p * 2^k
-    return x < -700.0 ? 0.0 : r;
+    const double kd = kt - MAGIC;
+    double r = fma(kd, -6.93147180369123816490e-01, x);
+    r = fma(kd, -1.90821492927058770002e-10, r);
+    double p = 1.0 / 3628800.0;
+    p = fma(p, r, 1.0 / 362880.0);
+    p = fma(p, r, 1.0 / 40320.0);
+    p = fma(p, r, 1.0 / 5040.0);
+    p = fma(p, r, 1.0 / 720.0);
+    p = fma(p, r, 1.0 / 120.0);
+    p = fma(p, r, 1.0 / 24.0);
+    p = fma(p, r, 1.0 / 6.0);
+    p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);
+    p = fma(p, r, 1.0);                                                // e^r in [0.707, 1.415]
+    const double v = __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));      // * 2^k
+    return x < -700.0 ? 0.0 : v;
+}
+
+// ln x for the rate table (x = T >= 1 K or 1 + u >= 1: normal, positive), 1e-13 absolute: x = 2^e m with m in [0.707, 1.414],
+// s = (m - 1)/(m + 1) from the hardware reciprocal seed and two Newton steps, ln m = 2 s (1 + s^2/3 + ... + s^14/15).
+// 27 instructions against the ~40 of the library's log (denormals, NaN, infinities).
+__device__ __forceinline__ double log_table(double x)
+{
+    int hi = __double2hiint(x);
+    int e = (hi >> 20) - 1023;
+    hi = (hi & 0x000fffff) | 0x3ff00000;
+    const bool up = hi > 0x3ff6a09e;                                   // m > sqrt(2): use m / 2
+    if (up) { hi -= 0x00100000; e += 1; }
+    const double m = __hiloint2double(hi, __double2loint(x));
+    const double f = m - 1.0, d = m + 1.0;
+    double rc;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc) : "d"(d));             // ~20 bits; d in [1.7, 2.42]
+    rc = fma(fma(-d, rc, 1.0), rc, rc);
+    rc = fma(fma(-d, rc, 1.0), rc, rc);
+    const double sq = f * rc, s2 = sq * sq;
+    double p = 1.0 / 15.0;
+    p = fma(p, s2, 1.0 / 13.0);
+    p = fma(p, s2, 1.0 / 11.0);
+    p = fma(p, s2, 1.0 / 9.0);
+    p = fma(p, s2, 1.0 / 7.0);
+    p = fma(p, s2, 1.0 / 5.0);
+    p = fma(p, s2, 1.0 / 3.0);
+    p = fma(p, s2, 1.0);
+    return fma((double)e, 0.693147180559945309417, 2.0 * sq * p);
 }
 
 template <bool FAST> struct RtMath;
-template <> struct RtMath<false> { static __device__ __forceinline__ double ex(double x) { return exp(x); } };
-template <> struct RtMath<true> { static __device__ __forceinline__ double ex(double x) { return exp_sfu(x); } };
+template <> struct RtMath<false> {
+    static __device__ __forceinline__ double ex(double x) { return exp(x); }
+    static __device__ __forceinline__ double lg(double x) { return log(x); }
+};
+template <> struct RtMath<true> {
+    static __device__ __forceinline__ double ex(double x) { return exp_table(x); }
+    static __device__ __forceinline__ double lg(double x) { return log_table(x); }
+};
 
-// FAST (fp32-field runs): the exponentials of the fits from exp_sfu; the logarithms stay fp64 (they sit in exponents: an
-// absolute error of 2e-7 there would be a relative error of up to 1e-6 in the rate)
+// FAST (the sub-cycled kernel, where the table is evaluated once per sub-cycle): the exponentials and logarithms of the fits
+// from exp_table / log_table.  The once-per-cell users (isothermal kernel, time step) keep the library's functions.
 template <bool FAST = false>
 __device__ __forceinline__ void rate_table(double T, const ChemK &q, Coef &k)
 {
     const double KB = 1.380649e-16;
     const double TR_H = 157807.0, TR_HE1 = 285335.0, TR_HE2 = 631515.0;   // ionisation thresholds in K
-    auto exp = [](double x) { return RtMath<FAST>::ex(x); };             // (shadows ::exp inside this function)
+    auto exp = [](double x) { return RtMath<FAST>::ex(x); };             // (these shadow ::exp and ::log inside this function)
+    auto log = [](double x) { return RtMath<FAST>::lg(x); };
     const double L = log(T), iT = 1.0 / T;
     // recombination and its cooling: A0 lambda^p / (1 + (lambda/l0)^q)^s
     const double ep = exp(-q.p_rec * L), eq = exp(-q.q_rec * L);
@@ -268,7 +312,7 @@ __global__ void __launch_bounds__(128, 5) arc_chem_kernel(long long ncell, doubl
         }
         if (__all_sync(0xffffffffu, mine < 0)) break;
         if (mine >= 0) {
-            if (c.t < dt && c.n < max_sub) chem_subcycle<false, sizeof(FT) == 4>(c, k, q, dt, eps, x_floor, max_sub);
+            if (c.t < dt && c.n < max_sub) chem_subcycle<false, true>(c, k, q, dt, eps, x_floor, max_sub);
             if (!(c.t < dt && c.n < max_sub)) {
                 xHIf[mine] = (FT)c.x0; xHeIf[mine] = (FT)c.x1; xHeIIf[mine] = (FT)c.x2; Tf[mine] = (FT)c.T;
                 my_sub += (unsigned long long)c.n;
