@@ -120,3 +120,48 @@ def test_config5_512_central_source_and_slab_chemistry():
         assert_close(a, b, R32, f"512^3 slab chemistry: {name}")
     assert sub.max() > 1
 
+
+
+def test_largest_grid_1024_cubed_per_ray_sequences():
+    """N = 1024 is the largest grid the library takes (10 bits per cell coordinate in the tracer, cell indices up to
+    2^30 - 1; the paper's production size): 12 root rays that never split (l0 = Lmax = 0) from a source next to
+    the far corner, so that rays run the whole length of the box through coordinates 0 and 1023 and through the highest cell
+    indices - per-ray cell sequences bit-exact against the oracle, accumulators and rates within the fp32 bar.  One bin,
+    fp32 fields: 96 GB of the 180 GB on the device."""
+    import dataclasses
+    import torch
+    from gpu_common import gpu_raylog_to_dict
+    N = 1024
+    n = N ** 3
+    w0 = wl.config2(8, dtype="f32")
+    box = w0.box_cm
+    pos = (np.array([[1000, 1010, 1021]]) + 0.5) * (box / N)
+    w = dataclasses.replace(w0, name="grid1024", N=N, n_H=np.full(n, 1e-3, np.float32), x_HI=np.full(n, 2e-2, np.float32),
+                            x_HeI=np.ones(n, np.float32), x_HeII=np.zeros(n, np.float32), T=np.full(n, 1e4, np.float32),
+                            src_pos_cm=pos, params=dict(w0.params, l0=0, Lmax=0, tau_term=float("inf")))
+    w.x_HI[:: 7] = 0.5                                             # (not uniform: every 7th cell is 25 times as opaque)
+    Ao, so, rl = orc.trace(w, log=True, cap_rays=64, cap_cells=100_000)
+    want = orc.raylog_to_dict(rl)
+    assert so["rays"] == 12 and so["segments"] > 3000 and max(len(c) for c, _ in want.values()) > 2000
+    cells = np.concatenate([np.array(c) for c, _ in want.values()])
+    assert cells.max() > 2 ** 30 - 2 ** 21 and cells.min() < 2 ** 27     # both ends of the index range are visited
+    with arc.Context(w, digest=1) as cx:
+        key, seq, cell = cx.trace_debug(cap=int(so["segments"] + so["rays"]) + 16)
+        st = cx.stats()
+        A = torch.empty((n, 1), dtype=torch.float64, device="cuda")
+        arc.arc_get_accum(cx.ctx, A)
+        G = torch.empty(n, dtype=torch.float64, device="cuda")
+        arc.arc_get_rates(cx.ctx, Gamma_HI=G)
+    assert gpu_raylog_to_dict(key, seq, cell) == want
+    compare_trace_stats(st, so, 1, R32)
+    hit = np.unique(cells)
+    A_h = A[:, 0].cpu().numpy()
+    assert_close(A_h[hit], Ao[hit, 0], R32, "1024^3: A in the visited cells")
+    assert np.count_nonzero(A_h) == np.count_nonzero(Ao[:, 0]) == len(hit)
+    V = (box / N) ** 3
+    G_want = Ao[hit, 0] / (V * (w.n_H[hit].astype(np.float64) * w.x_HI[hit].astype(np.float64)))     # Eq. 1, one absorber, one bin
+    assert_close(G.cpu().numpy()[hit], G_want, R32, "1024^3: Gamma_HI in the visited cells")
+    for bad in (1025, 2048):
+        with pytest.raises(arc.ArcError) as e:
+            arc.arc_create_grid(bad, box, arc.ARC_F32)
+        assert e.value.code == arc.ARC_EINVAL
