@@ -157,7 +157,8 @@ def test_largest_grid_1024_cubed_per_ray_sequences():
     hit = np.unique(cells)
     A_h = A[:, 0].cpu().numpy()
     assert_close(A_h[hit], Ao[hit, 0], R32, "1024^3: A in the visited cells")
-    assert np.count_nonzero(A_h) == np.count_nonzero(Ao[:, 0]) == len(hit)
+    # nothing outside the visited cells (a visited cell may hold exactly 0: the tied diagonal rays cross it in a zero-length segment)
+    assert np.count_nonzero(A_h) == np.count_nonzero(Ao[:, 0]) <= len(hit) and np.count_nonzero(A_h[hit]) == np.count_nonzero(A_h)
     V = (box / N) ** 3
     G_want = Ao[hit, 0] / (V * (w.n_H[hit].astype(np.float64) * w.x_HI[hit].astype(np.float64)))     # Eq. 1, one absorber, one bin
     assert_close(G.cpu().numpy()[hit], G_want, R32, "1024^3: Gamma_HI in the visited cells")
