@@ -1,0 +1,109 @@
+"""Seeded random sweep of the tracer's parameter space against the oracle (through the C ABI): grid size, source count
+and placement (cell centres, faces, arbitrary), bin count, field dtype, start level, maximum level, rays per cell, tau_term,
+opacity scale, deposit route, geometric-correction mode, emission masks, persistent-grid size.  Every case compares the
+per-ray cell sequences and end reasons (bit-exact), all integer tallies and the traversal digest (bit-exact), the float
+tallies and every accumulator (1e-5 fp64 fields / 1e-3 fp32 fields).  The fixed cases of tests/test_gpu_parity.py and
+tests/test_gpu_geom.py were chosen by hand; this sweep is there for the combinations nobody thought of."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_1807_07094_b200 import arc, workloads as wl
+from gpu_common import RTOL, assert_close, compare_trace_stats, gpu_raylog_to_dict
+
+pytestmark = pytest.mark.gpu
+
+import os
+
+N_CASES = int(os.environ.get("ARC_FUZZ_CASES", "400"))        # (a multiple of 8; ARC_FUZZ_CASES=4000 for a long sweep)
+N_CHEM = int(os.environ.get("ARC_FUZZ_CHEM_CASES", "80"))     # (a multiple of 4)
+
+
+def _case(i):
+    rng = np.random.default_rng(180707094 * 31 + i)
+    N = int(rng.choice([1, 2, 3, 5, 8, 11, 16, 24, 33]))
+    nb = int(rng.integers(1, 9))
+    dtype = "f32" if rng.random() < 0.5 else "f64"
+    nsrc = int(rng.choice([1, 1, 2, 3, 7, 20]))
+    l0 = int(rng.choice([0, 0, 1, 1, 2]))
+    w = wl.tiny(N=N, nsrc=nsrc, nb=nb, seed=1000 + i, dtype=dtype, l0=l0, Yp=float(rng.choice([0.0, 0.24])),
+                kappa_scale=float(10.0 ** rng.uniform(-1.0, 2.5)), off_centre=bool(rng.random() < 0.6))
+    place = rng.random()
+    dx = w.box_cm / N
+    if place < 0.25:                                   # sources exactly on faces / edges / corners of cells
+        w.src_pos_cm = rng.integers(0, N, (nsrc, 3)).astype(np.float64) * dx
+    elif place < 0.35:                                 # next to the upper box faces
+        w.src_pos_cm = np.minimum((N - rng.random((nsrc, 3)) * 0.01) * dx, np.nextafter(w.box_cm, 0.0) * (1 - 1e-12))
+    over = dict(Phi=float(rng.choice([1.0, 3.0, 3.0, 5.5])), Lmax=int(rng.choice([l0, l0 + 1, 5, 13])),
+                tau_term=float(rng.choice([0.3, 3.0, 30.0, math.inf])))
+    geom = int(rng.choice([0, 0, 1, 2, 2, 3]))
+    dep = arc.ARC_DEPOSIT_AUTO if geom else int(rng.choice([arc.ARC_DEPOSIT_AUTO, arc.ARC_DEPOSIT_RED, arc.ARC_DEPOSIT_AGG, arc.ARC_DEPOSIT_QUAD]))
+    blocks = int(rng.choice([0, 0, 1, 2, 5]))
+    mask = None
+    if rng.random() < 0.3:
+        mask = (rng.random((nsrc, 12 << (2 * l0))) < rng.uniform(0.1, 0.9)).astype(np.uint8)
+    return w, over, geom, dep, blocks, mask
+
+
+@pytest.mark.parametrize("chunk", range(8))
+def test_random_cases_against_the_oracle(chunk):
+    for i in range(chunk * (N_CASES // 8), (chunk + 1) * (N_CASES // 8)):
+        w, over, geom, dep, blocks, mask = _case(i)
+        what = f"case {i}: N={w.N} nsrc={w.nsrc} nb={w.nb} {w.dtype} l0={w.params['l0']} {over} geom={geom} deposit={dep} blocks={blocks} mask={mask is not None}"
+        try:
+            Ao, so, rl = orc.trace(w, log=True, blocked=mask, geom_corr=geom, **over)
+            want = orc.raylog_to_dict(rl)
+            with arc.Context(w, digest=1, geom_corr=geom, deposit=dep, trace_blocks=blocks, **over) as cx:
+                if mask is not None:
+                    cx.set_emission_mask(mask)
+                key, seq, cell = cx.trace_debug(cap=int(so["segments"] + so["rays"]) + 64)
+                st = cx.stats()
+                A = cx.accum()
+                cx.trace()                              # the non-logging variant of the same configuration
+                st2 = cx.stats()
+                A2 = cx.accum()
+            assert gpu_raylog_to_dict(key, seq, cell) == want, "per-ray cell sequences / end reasons differ"
+            for s_, A_ in ((st, A), (st2, A2)):
+                if geom in (1, 3):                      # f_c alone loses photons by design: `absorbed` is what was deposited
+                    assert s_["segments"] == so["segments"] and s_["digest"] == so["digest"] and np.array_equal(s_["ends"], so["ends"])
+                    assert_close(s_["absorbed"], so["absorbed"], RTOL[w.dtype], "absorbed")
+                else:
+                    compare_trace_stats(s_, so, w.nb, RTOL[w.dtype])
+                assert_close(A_, Ao, RTOL[w.dtype], "A")
+        except AssertionError as e:
+            raise AssertionError(f"{what}\n{e}") from None
+
+
+@pytest.mark.parametrize("chunk", range(4))
+def test_random_chemistry_cases_against_the_oracle(chunk):
+    """the per-cell update over random states, rates, time steps and switches (field dtype, isothermal, case A / B,
+    collisional ionisation, helium abundance, sub-cycle cap and eps): the device's rates are handed to the oracle, every
+    cell must agree within the bar, the sub-cycle totals to 1e-4"""
+    for i in range(chunk * (N_CHEM // 4), (chunk + 1) * (N_CHEM // 4)):
+        rng = np.random.default_rng(180707094 * 37 + i)
+        dtype = "f32" if rng.random() < 0.5 else "f64"
+        nb = int(rng.integers(1, 6))
+        w = wl.tiny(N=int(rng.choice([6, 9, 12])), nsrc=int(rng.choice([1, 3])), nb=nb, seed=2000 + i, dtype=dtype,
+                    Yp=float(rng.choice([0.0, 0.1, 0.24])), kappa_scale=float(10.0 ** rng.uniform(0.0, 1.5)))
+        w.src_Ndot = w.src_Ndot * float(10.0 ** rng.uniform(0.0, 5.0))
+        over = dict(isothermal=int(rng.random() < 0.3), caseB=int(rng.random() < 0.5), coll_ion=int(rng.random() < 0.7),
+                    max_subcycles=int(rng.choice([1, 7, 300, 4096])), eps_sub=float(rng.choice([0.05, 0.1, 0.3])))
+        dt = w.dt_s * float(10.0 ** rng.uniform(-2.0, 1.5))
+        what = f"chemistry case {i}: N={w.N} nb={nb} {dtype} Yp={w.params['Yp']} {over} dt={dt:.3e}"
+        try:
+            with arc.Context(w, **over) as cx:
+                cx.trace()
+                G, H, _ = cx.rates()
+                cx.update_chemistry(dt)
+                got = cx.get_fields()
+                st = cx.stats()
+            want, sub = orc.chemistry(w, w.fields(), G, H, dt, **over)
+            for n, a, b in zip(("x_HI", "x_HeI", "x_HeII", "T"), got[1:], want[1:]):
+                assert_close(a, b, RTOL[dtype], n)
+            tot = int(sub.sum())
+            assert abs(st["subcycles"] - tot) <= max(4, tot // 10000), (st["subcycles"], tot)
+            assert st["max_subcycles_cell"] == int(sub.max())
+        except AssertionError as e:
+            raise AssertionError(f"{what}\n{e}") from None
