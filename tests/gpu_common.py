@@ -52,7 +52,12 @@ def compare_trace_stats(gs, os_, nb, rtol, check_digest=True):
         assert gs["digest"] == os_["digest"], f"traversal digest {gs['digest']:#x} vs {os_['digest']:#x}"
     assert_close(gs["emitted"], os_["emitted"], 1e-14, "emitted")
     assert_close(gs["absorbed"], os_["absorbed"], max(rtol * 1e-2, 1e-9), "absorbed")
-    assert_close(gs["escaped"], os_["escaped"], rtol, "escaped", atol_frac=0.0 if False else 1e-12)
+    # escaped: the protocol's absolute floor is 1e-12 of the array's scale - for the photon tallies that scale is what
+    # the sources emit (an opaque box lets e^-hundreds of it out: 1e-68 against 0 is not a difference)
+    scale = float(np.max(np.abs(os_["emitted"]))) if len(os_["emitted"]) else 0.0
+    e_g, e_o = np.asarray(gs["escaped"], dtype=np.float64), np.asarray(os_["escaped"], dtype=np.float64)
+    bad = np.abs(e_g - e_o) > rtol * np.maximum(np.abs(e_g), np.abs(e_o)) + 1e-12 * scale
+    assert not bad.any(), f"escaped: gpu={e_g} oracle={e_o} (emitted {os_['emitted']})"
 
 
 def run_gpu_trace(w, fields=None, **override):

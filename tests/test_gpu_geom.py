@@ -48,9 +48,7 @@ def test_axis_ray_closed_form_on_the_gpu():
     f = lambda k: 1.0 if 1.0 >= k * w0 else 0.5 + 0.5 / (k * w0)
     for k in range(2, N - c - 1):
         expect = f(k) * a(k) + (1 - f(k + 1)) * a(k + 1)
-        # 1e-6: the CUDA path takes the quotient D_edge / L_pix of Eq. 2 in fp32 (it weighs the deposit, it decides
-        # nothing: DESIGN.md 6.2 step 7) - a tenth of the fp64 parity bar of 1e-5
-        assert abs(A[c, c, c + k] - expect) <= 1e-6 * expect, k
+        assert abs(A[c, c, c + k] - expect) <= 1e-9 * expect, k
 
 
 def test_config1_steps_with_the_papers_correction():
