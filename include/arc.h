@@ -251,6 +251,21 @@ int arc_pix2vec(const int32_t *level, const uint32_t *pix, int n, double *out);
  * __ddiv_rn(a, d).  *mismatches must come back 0.  HOST pointer; synchronises; default stream. */
 int arc_selftest_division(uint64_t n_pairs, uint64_t seed, uint64_t *mismatches);
 
+/* arc_pix2vec for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): same arguments, same results to the bit, but the device staging that arc_pix2vec cudaMalloc's and
+ * cudaFree's on every call lives in ONE file-scope device array of fixed size (csrc/arc_noalloc.cu), so the call makes no
+ * cudaMalloc, no cudaFree and no allocating library call.  Limit: n <= ARC_PIX2VEC_NOALLOC_MAX = 4096 pairs per call
+ * (128 KiB of device memory, held by every GPU that loads the library until the process exits); more is ARC_EINVAL with
+ * the reason in arc_noalloc_last_error() - split the call.  HOST pointers; out is [n][3]; synchronous on the legacy
+ * default stream of the current device.  All calls on a device share the array and it keeps the last call's contents
+ * (nothing in it needs to start at zero: the n inputs are overwritten before they are read, the 3 n outputs written
+ * before they are copied back); calls through this entry point are serialised by a mutex, anything else that touched
+ * the array concurrently on the GPU would race.  Errors: ARC_EINVAL (NULL, n < 0, n > max, not a pixel), ARC_ECUDA. */
+#define ARC_PIX2VEC_NOALLOC_MAX 4096
+int arc_pix2vec_noalloc(const int32_t *level, const uint32_t *pix, int n, double *out);
+int arc_pix2vec_noalloc_max(void);                     /* = ARC_PIX2VEC_NOALLOC_MAX of the loaded library */
+const char *arc_noalloc_last_error(void);              /* text of this thread's last arc_pix2vec_noalloc failure */
+
 const char *arc_last_error(const arc_ctx *c);          /* c may be NULL: last error of a failed create */
 const char *arc_version(void);
 

@@ -32,7 +32,8 @@ EXPORTS = ["arc_create_grid", "arc_destroy", "arc_default_params", "arc_set_para
            "arc_set_fields", "arc_get_fields", "arc_set_spectrum", "arc_set_sources", "arc_set_emission_mask", "arc_get_thin_radii", "arc_set_thin_radii", "arc_trace",
            "arc_trace_partial", "arc_accum_device", "arc_finalize",
            "arc_get_rates", "arc_get_accum", "arc_update_chemistry", "arc_run_steps", "arc_suggest_dt", "arc_synchronize", "arc_get_stats",
-           "arc_trace_debug", "arc_pix2vec", "arc_selftest_division", "arc_last_error", "arc_version"]
+           "arc_trace_debug", "arc_pix2vec", "arc_selftest_division", "arc_pix2vec_noalloc", "arc_pix2vec_noalloc_max",
+           "arc_noalloc_last_error", "arc_last_error", "arc_version"]
 
 
 class ArcError(RuntimeError):
@@ -110,6 +111,9 @@ def lib():
         l.arc_trace_debug.argtypes = [vp, i32, C.POINTER(arc_raylog)]
         l.arc_pix2vec.argtypes = [vp, vp, i32, vp]
         l.arc_selftest_division.argtypes = [C.c_uint64, C.c_uint64, C.POINTER(C.c_uint64)]
+        l.arc_pix2vec_noalloc.argtypes = [vp, vp, i32, vp]
+        l.arc_pix2vec_noalloc_max.restype = i32
+        l.arc_noalloc_last_error.restype = C.c_char_p
         l.arc_last_error.argtypes = [vp]
         l.arc_last_error.restype = C.c_char_p
         l.arc_version.restype = C.c_char_p
@@ -314,6 +318,29 @@ def arc_pix2vec(level, pix) -> np.ndarray:
     rc = lib().arc_pix2vec(C.c_void_p(lv.ctypes.data), C.c_void_p(px.ctypes.data), len(lv), C.c_void_p(out.ctypes.data))
     if rc != ARC_OK:
         raise ArcError(rc, "arc_pix2vec failed")
+    return out
+
+
+def arc_pix2vec_noalloc_max() -> int:
+    return int(lib().arc_pix2vec_noalloc_max())
+
+
+def arc_noalloc_last_error() -> str:
+    return (lib().arc_noalloc_last_error() or b"").decode()
+
+
+def arc_pix2vec_noalloc(level, pix, out=None) -> np.ndarray:
+    """arc_pix2vec without any device allocation (fixed 128 KiB device scratch; at most arc_pix2vec_noalloc_max() pairs
+    per call).  `out` (float64 [n, 3], C order) may be passed in so that the host side allocates nothing either."""
+    lv = np.ascontiguousarray(np.asarray(level, dtype=np.int32))
+    px = np.ascontiguousarray(np.asarray(pix, dtype=np.uint32))
+    if out is None:
+        out = np.zeros((len(lv), 3))
+    if out.dtype != np.float64 or not out.flags["C_CONTIGUOUS"] or out.size < 3 * len(lv):
+        raise ValueError("out must be a C-contiguous float64 array of at least 3 n values")
+    rc = lib().arc_pix2vec_noalloc(C.c_void_p(lv.ctypes.data), C.c_void_p(px.ctypes.data), len(lv), C.c_void_p(out.ctypes.data))
+    if rc != ARC_OK:
+        raise ArcError(rc, arc_noalloc_last_error())
     return out
 
 
